@@ -1,0 +1,151 @@
+/* pic_b200.h — C ABI of the B200-native PIC particle step.
+ *
+ * One call = one piece of the per-supercell particle step of an electromagnetic
+ * particle-in-cell code on a staggered Yee grid (§3.1 "PIConGPU";
+ * the call list is BASELINE.json:north_star, the definitions SURVEY.md §8(c) steps 1-7):
+ *
+ *     gather E,B at x^n (CIC/TSC/PQS)  ->  relativistic Boris push  ->  move
+ *     ->  charge-conserving Esirkepov deposit of J  ->  resort across supercells.
+ *
+ * Conventions (readings S1-S22): c = 1; u = gamma*v/c;
+ * du/dt = (q/m)(E + v x B); all boundaries periodic; leapfrog time centring (the
+ * loaded u is u^{n-1/2}); J is zeroed at the start of every step, so after
+ * pic_step(n) it holds the current of the LAST step.
+ *
+ * Memory.  Every pointer is a DEVICE pointer unless the argument says "host".
+ * The caller owns everything it passes.  The library owns no device memory of its
+ * own: all of its state lives inside ONE caller-provided device workspace
+ * (pic_workspace_bytes() -> size; allocate it e.g. as a torch uint8 tensor, 256-byte
+ * aligned; hand it to pic_create; free it after pic_destroy).  All work is enqueued
+ * on the cudaStream_t given to pic_create; calls that return host values
+ * (pic_get_particles' n_out, pic_get_counts to a host buffer is NOT offered —
+ * see each call) synchronise that stream, the others are asynchronous.
+ *
+ * Array layout.  Grid arrays (E, B, J components) are float32 of nx*ny*nz elements,
+ * index i + nx*(j + ny*k), each component sampled at its Yee location
+ * (SURVEY.md §8(c) step 2): Ex,Jx @ (i+1/2,j,k); Ey,Jy @ (i,j+1/2,k); Ez,Jz @ (i,j,k+1/2);
+ * Bx @ (i,j+1/2,k+1/2); By @ (i+1/2,j,k+1/2); Bz @ (i+1/2,j+1/2,k).
+ * Particle arrays are structure-of-arrays, one element per particle.
+ *
+ * Errors.  Every call returns 0 (PIC_OK) or a negative code; no exception crosses
+ * the ABI.  pic_last_error(ctx) returns a static/owned human-readable string for
+ * the last failing call on that context.  Faults detected on the device (frame pool
+ * or exchange buffer exhausted, a particle moving >= 1 cell) set a sticky error word
+ * that the next synchronising call (pic_get_*, pic_sync) reports as PIC_EDEVICE.
+ */
+#ifndef PIC_B200_H
+#define PIC_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PIC_OK        0
+#define PIC_EINVAL   -1   /* bad argument (dims, order, c*dt >= cell, NULL, ...) */
+#define PIC_ENOMEM   -2   /* workspace too small / capacity exceeded */
+#define PIC_ECUDA    -3   /* a CUDA runtime or driver call failed */
+#define PIC_ESTATE   -4   /* call out of order (step before fields / particles) */
+#define PIC_EDEVICE  -5   /* sticky device-side fault, see pic_get_stats()[7] */
+
+#define PIC_MAX_SPECIES 16
+
+/* bits of the sticky device error word (pic_get_stats()[7]) */
+#define PIC_DEV_FRAME_POOL_EXHAUSTED   1
+#define PIC_DEV_EXCHANGE_OVERFLOW      2
+#define PIC_DEV_TABLE_POOL_EXHAUSTED   4
+#define PIC_DEV_MOVED_TOO_FAR          8
+#define PIC_DEV_TMA_TIMEOUT           16
+
+typedef struct pic_ctx pic_ctx;   /* opaque, host-side */
+
+/* Size in bytes of the device workspace pic_create needs for this geometry and
+ * particle capacity.  grid[3] = cells per axis (each a multiple of supercell[a]);
+ * supercell[3] = supercell extent in cells (must be {8,8,4}: the tile sizes are
+ * compile-time); shape_order 1 CIC, 2 TSC, 3 PQS (S2);
+ * max_particles = capacity over the life of the context.  host pointers. */
+int32_t pic_workspace_bytes(const int32_t grid[3], const int32_t supercell[3],
+                            int32_t shape_order, int64_t max_particles, uint64_t* bytes_out);
+
+/* Create a context (BASELINE.json:north_star "pic_create(grid dims, cell size, dt,
+ * supercell dims, shape order)").  cell[3] = cell size, dt = time step, both in units
+ * with c = 1; requires dt < min(cell) so no particle moves a full cell per step
+ * (SURVEY.md §8(c) step 5).  workspace = device memory of >= pic_workspace_bytes()
+ * bytes, 256-byte aligned, zero-initialisation not required; stream = cudaStream_t
+ * (0 = legacy default stream).  grid/cell/supercell are host pointers. */
+int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], double dt,
+                   const int32_t supercell[3], int32_t shape_order, int64_t max_particles,
+                   void* workspace, uint64_t workspace_bytes, void* stream);
+
+/* Species table (reading S15): charge q[s] and mass m[s], host pointers, n <=
+ * PIC_MAX_SPECIES.  Default for every species id: q = -1, m = 1. */
+int32_t pic_set_species(pic_ctx* ctx, int32_t n, const double* q, const double* m);
+
+/* Append n particles ("pic_load_particles(SoA x/u/weight/species)").  x,y,z: float64
+ * global positions in the units of cell[], anywhere (wrapped periodically into
+ * [0, N*cell)); stored internally as (cell index, fp32 in-cell fraction) — exact
+ * when x/cell is an integer plus an fp32 fraction.  ux,uy,uz: float32 gamma*beta at
+ * t^{n-1/2} (S4).  w: float32 weight.  species: int32 in [0, PIC_MAX_SPECIES) or
+ * NULL (= all 0).  Particle ids are the load order, starting at 0 and continuing
+ * across calls.  Asynchronous on the stream; the arrays must stay valid until the
+ * stream reaches this point. */
+int32_t pic_load_particles(pic_ctx* ctx, int64_t n,
+                           const double* x, const double* y, const double* z,
+                           const float* ux, const float* uy, const float* uz,
+                           const float* w, const int32_t* species);
+
+/* Set the static external fields ("pic_set_fields(E,B)"): six float32 grid arrays,
+ * copied into the workspace (asynchronous). */
+int32_t pic_set_fields(pic_ctx* ctx, const float* Ex, const float* Ey, const float* Ez,
+                       const float* Bx, const float* By, const float* Bz);
+
+/* Advance n steps ("pic_step(n)"); asynchronous.  Each step, per supercell:
+ * stage the E/B tile + guards in shared memory, gather, Boris push, move,
+ * Esirkepov deposit into a shared-memory J tile flushed once to global J, and
+ * resort of particles that changed supercell. */
+int32_t pic_step(pic_ctx* ctx, int32_t n);
+
+/* Copy the last step's J ("pic_get_current"), periodic-folded, three float32 grid
+ * arrays (any may be NULL).  Asynchronous device-to-device copy on the stream. */
+int32_t pic_get_current(pic_ctx* ctx, float* Jx, float* Jy, float* Jz);
+
+/* Read particles back ("pic_get_particles"), supercell-major order (S21: match by
+ * id).  capacity = elements available in each non-NULL array; *n_out (host) = number
+ * of particles (written even if capacity is too small, in which case PIC_ENOMEM).
+ * x,y,z float64 = (cell + fraction)*cell size; supercell = linear index
+ * sx + nsx*(sy + nsy*sz) of the frame list holding the particle.  Synchronises. */
+int32_t pic_get_particles(pic_ctx* ctx, int64_t capacity, int64_t* n_out,
+                          double* x, double* y, double* z,
+                          float* ux, float* uy, float* uz, float* w,
+                          int32_t* species, uint32_t* id, int32_t* supercell);
+
+/* Per-supercell particle counts, int32[nsx*nsy*nsz] on the DEVICE.  Asynchronous. */
+int32_t pic_get_counts(pic_ctx* ctx, int32_t* per_supercell_count);
+
+/* stats (host int64[8]): [0] particles, [1] supercell-leavers of the last step,
+ * [2] frames in use, [3] frames in the pool, [4] max particles in one supercell,
+ * [5] steps done, [6] cumulative leavers, [7] sticky device error word.
+ * Synchronises; returns PIC_EDEVICE if [7] != 0. */
+int32_t pic_get_stats(pic_ctx* ctx, int64_t stats[8]);
+
+/* Wait for the stream and report a sticky device error, if any. */
+int32_t pic_sync(pic_ctx* ctx);
+
+/* Kernel variant switches for measurement (all variants compute the same step):
+ * key "tma" (1 = stage E/B tiles with cp.async.bulk.tensor, 0 = plain loads),
+ * key "graph" (1 = replay pic_step through a CUDA graph).  Host strings. */
+int32_t pic_set_option(pic_ctx* ctx, const char* key, int64_t value);
+
+/* Number of kernel launches enqueued by this context so far (host counter). */
+int64_t pic_launch_count(const pic_ctx* ctx);
+
+const char* pic_last_error(const pic_ctx* ctx);   /* ctx may be NULL: last create error */
+
+int32_t pic_destroy(pic_ctx* ctx);                /* frees host state only */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PIC_B200_H */

@@ -1,0 +1,575 @@
+// pic_api.cu — the C ABI of include/pic_b200.h: context, workspace carving, particle
+// load / read-back, field upload.  The step itself is in pic_step.cu.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <cuda.h>
+
+#include <new>
+#include <string>
+
+#include "../../include/pic_b200.h"
+#include "pic_internal.cuh"
+
+struct pic_ctx {
+    PicDev d;
+    int order;
+    double cell[3], dt;
+    double q[PIC_NSPECIES], m[PIC_NSPECIES];
+    int64_t max_particles, n_particles, steps, launches;
+    cudaStream_t stream;
+    bool have_fields;
+    bool use_tma, use_graph;
+    char* ws;
+    uint64_t ws_bytes;
+    std::string err;
+    // TMA descriptor + graph cache (pic_tma.cu / pic_api.cu)
+    alignas(64) unsigned char tmap[128];
+    bool tmap_ok;
+    cudaGraphExec_t graph_exec;
+    int graph_steps;
+};
+
+static std::string g_create_error;
+
+// ------------------------------------------------------------------ workspace layout
+namespace {
+
+struct Layout {
+    uint64_t pos, mom, pid, tbl_pool, tbl_off, tbl_cap, sc_nframes, sc_count, sc_stay, sc_incoming,
+        x_pos, x_mom, x_id, x_dst, ctr, ctr64, F, Fpad, J, sc_offset, total;
+    int n_frames, tbl_pool_size, x_cap, nsc;
+};
+
+uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
+
+int compute_layout(const int32_t grid[3], const int32_t sc[3], int order, int64_t maxp, Layout* L)
+{
+    if (!grid || !sc) return PIC_EINVAL;
+    if (sc[0] != PIC_SCX || sc[1] != PIC_SCY || sc[2] != PIC_SCZ) return PIC_EINVAL;
+    if (order < 1 || order > 3 || maxp < 0) return PIC_EINVAL;
+    for (int a = 0; a < 3; ++a)
+        if (grid[a] <= 0 || grid[a] % sc[a] != 0) return PIC_EINVAL;
+    const uint64_t nsc = (uint64_t)(grid[0] / sc[0]) * (grid[1] / sc[1]) * (grid[2] / sc[2]);
+    const uint64_t ncell = (uint64_t)grid[0] * grid[1] * grid[2];
+    if (nsc > (1u << 30) || (uint64_t)maxp > (1ull << 32) - 1) return PIC_EINVAL;
+    // every supercell may hold one partly filled frame; 1/8 head-room for density drift
+    const uint64_t n_frames = (uint64_t)maxp / PIC_FRAME + (uint64_t)maxp / (8 * PIC_FRAME) + 2 * nsc + 64;
+    const uint64_t slots = n_frames * PIC_FRAME;
+    const uint64_t tblp = 4 * n_frames + 16 * nsc + 1024;
+    uint64_t xcap = (uint64_t)maxp / 4 + 65536;
+    if (xcap > (uint64_t)maxp + 1024) xcap = (uint64_t)maxp + 1024;
+    if (n_frames > 0x7fffffffull / 2 || tblp > 0x7fffffffull || xcap > 0x7fffffffull) return PIC_EINVAL;
+    uint64_t o = 0;
+    auto take = [&](uint64_t bytes) { uint64_t r = o; o = align_up(o + bytes, 256); return r; };
+    L->pos = take(slots * 16);
+    L->mom = take(slots * 16);
+    L->pid = take(slots * 4);
+    L->tbl_pool = take(tblp * 4);
+    L->tbl_off = take(nsc * 4);
+    L->tbl_cap = take(nsc * 4);
+    L->sc_nframes = take(nsc * 4);
+    L->sc_count = take(nsc * 4);
+    L->sc_stay = take(nsc * 4);
+    L->sc_incoming = take(nsc * 4);
+    L->x_pos = take(xcap * 16);
+    L->x_mom = take(xcap * 16);
+    L->x_id = take(xcap * 4);
+    L->x_dst = take(xcap * 4);
+    L->ctr = take(CTR_N * 4);
+    L->ctr64 = take(CTR64_N * 8);
+    L->F = take(6 * ncell * 4);
+    L->Fpad = take(6ull * (grid[0] + PIC_PAD_X) * (grid[1] + PIC_PAD_Y) * (grid[2] + PIC_PAD_Z) * 4);
+    L->J = take(3 * ncell * 4);
+    L->sc_offset = take((nsc + 1) * 8);
+    L->total = o;
+    L->n_frames = (int)n_frames;
+    L->tbl_pool_size = (int)tblp;
+    L->x_cap = (int)xcap;
+    L->nsc = (int)nsc;
+    return PIC_OK;
+}
+
+int fail(pic_ctx* c, int code, const std::string& msg)
+{
+    if (c) c->err = msg; else g_create_error = msg;
+    return code;
+}
+
+int cuda_fail(pic_ctx* c, cudaError_t e, const char* what)
+{
+    return fail(c, PIC_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+// ------------------------------------------------------------------ load kernels
+// Position (float64, physical units) -> wrapped integer cell + fp32 in-cell fraction.
+__device__ __forceinline__ void split_position(double x, double inv_cell, int n, int& cell, float& frac)
+{
+    double X = x * inv_cell;
+    double c = floor(X);
+    float f = (float)(X - c);
+    if (f >= 1.0f) { f = 0.0f; c += 1.0; }
+    if (f < 0.0f) f = 0.0f;
+    double r = fmod(c, (double)n);
+    if (r < 0) r += (double)n;
+    cell = (int)r;
+    if (cell >= n) cell = 0;
+    frac = f;
+}
+
+struct LoadArgs {
+    const double *x, *y, *z;
+    const float *ux, *uy, *uz, *w;
+    const int32_t* species;
+    long long n;
+    unsigned id0;
+    double icx, icy, icz;
+};
+
+__device__ __forceinline__ int load_locate(const PicDev& d, const LoadArgs& a, long long i,
+                                           float4& P, int& lc)
+{
+    int cx, cy, cz;
+    float fx, fy, fz;
+    split_position(a.x[i], a.icx, d.nx, cx, fx);
+    split_position(a.y[i], a.icy, d.ny, cy, fy);
+    split_position(a.z[i], a.icz, d.nz, cz, fz);
+    P = make_float4(fx, fy, fz, a.w[i]);
+    lc = (cx % PIC_SCX) + PIC_SCX * ((cy % PIC_SCY) + PIC_SCY * (cz % PIC_SCZ));
+    return (cx / PIC_SCX) + d.nsx * ((cy / PIC_SCY) + d.nsy * (cz / PIC_SCZ));
+}
+
+__global__ void pic_load_count_kernel(const PicDev d, const LoadArgs a)
+{
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < a.n;
+         i += (long long)gridDim.x * blockDim.x) {
+        float4 P;
+        int lc;
+        int s = load_locate(d, a, i, P, lc);
+        atomicAdd(d.sc_incoming + s, 1);
+    }
+}
+
+__global__ void pic_load_scatter_kernel(const PicDev d, const LoadArgs a)
+{
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < a.n;
+         i += (long long)gridDim.x * blockDim.x) {
+        float4 P;
+        int lc;
+        const int s = load_locate(d, a, i, P, lc);
+        const int sp = a.species ? a.species[i] : 0;
+        const int slot = atomicAdd(d.sc_count + s, 1);
+        const int fr = slot >> 8;
+        if (fr < d.sc_nframes[s]) {
+            const size_t idx = (size_t)d.tbl_pool[d.tbl_off[s] + fr] * PIC_FRAME + (slot & (PIC_FRAME - 1));
+            d.pos[idx] = P;
+            d.mom[idx] = make_float4(a.ux[i], a.uy[i], a.uz[i],
+                                     __uint_as_float(pic_pack_bits(lc, sp & (PIC_NSPECIES - 1))));
+            d.pid[idx] = a.id0 + (unsigned)i;
+        }
+    }
+}
+
+__global__ void pic_copy_int_kernel(int* dst, const int* src, int n)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) dst[i] = src[i];
+}
+
+// ------------------------------------------------------------------ read-back kernels
+__global__ void pic_scan_counts_kernel(const PicDev d)
+{
+    __shared__ long long part[1024];
+    const int t = threadIdx.x;
+    const int per = (d.nsc + 1023) / 1024;
+    const int lo = min(t * per, d.nsc), hi = min(lo + per, d.nsc);
+    long long sum = 0;
+    for (int i = lo; i < hi; ++i) sum += d.sc_count[i];
+    part[t] = sum;
+    __syncthreads();
+    if (t == 0) {
+        long long run = 0;
+        for (int i = 0; i < 1024; ++i) { long long v = part[i]; part[i] = run; run += v; }
+        d.sc_offset[d.nsc] = run;
+    }
+    __syncthreads();
+    long long run = part[t];
+    for (int i = lo; i < hi; ++i) { d.sc_offset[i] = run; run += d.sc_count[i]; }
+}
+
+struct GetArgs {
+    double *x, *y, *z;
+    float *ux, *uy, *uz, *w;
+    int32_t* species;
+    uint32_t* id;
+    int32_t* supercell;
+    long long capacity;
+    double cx, cy, cz;
+};
+
+__global__ void pic_get_particles_kernel(const PicDev d, const GetArgs a)
+{
+    const int s = blockIdx.x;
+    const int count = d.sc_count[s];
+    const long long off = d.sc_offset[s];
+    const int* tbl = d.tbl_pool + d.tbl_off[s];
+    const int ox = (s % d.nsx) * PIC_SCX, oy = ((s / d.nsx) % d.nsy) * PIC_SCY, oz = (s / (d.nsx * d.nsy)) * PIC_SCZ;
+    for (int slot = threadIdx.x; slot < count; slot += blockDim.x) {
+        const long long o = off + slot;
+        if (o >= a.capacity) break;
+        const size_t idx = (size_t)tbl[slot >> 8] * PIC_FRAME + (slot & (PIC_FRAME - 1));
+        const float4 P = d.pos[idx];
+        const float4 M = d.mom[idx];
+        const uint32_t bits = __float_as_uint(M.w);
+        const int lc = bits & 0xffff;
+        if (a.x) a.x[o] = ((double)(ox + (lc & 7)) + (double)P.x) * a.cx;
+        if (a.y) a.y[o] = ((double)(oy + ((lc >> 3) & 7)) + (double)P.y) * a.cy;
+        if (a.z) a.z[o] = ((double)(oz + (lc >> 6)) + (double)P.z) * a.cz;
+        if (a.ux) a.ux[o] = M.x;
+        if (a.uy) a.uy[o] = M.y;
+        if (a.uz) a.uz[o] = M.z;
+        if (a.w) a.w[o] = P.w;
+        if (a.species) a.species[o] = (bits >> 16) & 0xff;
+        if (a.id) a.id[o] = d.pid[idx];
+        if (a.supercell) a.supercell[o] = s;
+    }
+}
+
+// Padded copy of the fields with periodic halos (source of the TMA tile loads).
+__global__ void pic_pad_fields_kernel(const PicDev d, float* dst)
+{
+    const int px = d.nx + PIC_PAD_X, py = d.ny + PIC_PAD_Y, pz = d.nz + PIC_PAD_Z;
+    const size_t n = (size_t)6 * px * py * pz;
+    const size_t ncell = (size_t)d.nx * d.ny * d.nz;
+    for (size_t e = blockIdx.x * (size_t)blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+        size_t r = e;
+        int i = (int)(r % px); r /= px;
+        int j = (int)(r % py); r /= py;
+        int k = (int)(r % pz);
+        int c = (int)(r / pz);
+        int gi = ((i - PIC_PAD_LO) % d.nx + d.nx) % d.nx;
+        int gj = ((j - PIC_PAD_LO) % d.ny + d.ny) % d.ny;
+        int gk = ((k - PIC_PAD_LO) % d.nz + d.nz) % d.nz;
+        dst[e] = d.F[c * ncell + (size_t)gi + (size_t)d.nx * ((size_t)gj + (size_t)d.ny * gk)];
+    }
+}
+
+void refresh_species(pic_ctx* c)
+{
+    for (int s = 0; s < PIC_NSPECIES; ++s) {
+        c->d.h[s] = (float)((c->q[s] / c->m[s]) * c->dt * 0.5);
+        c->d.q[s] = (float)c->q[s];
+    }
+}
+
+int check_device(pic_ctx* c)
+{
+    int err = 0;
+    cudaError_t e = cudaMemcpyAsync(&err, c->d.ctr + CTR_ERROR, sizeof(int), cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "reading the device error word");
+    if (err) {
+        char buf[160];
+        snprintf(buf, sizeof buf, "device fault word 0x%x (1 frame pool, 2 exchange buffer, 4 table pool, 8 moved >= 1 cell, 16 TMA timeout)", err);
+        return fail(c, PIC_EDEVICE, buf);
+    }
+    return PIC_OK;
+}
+
+}  // namespace
+
+// 4-D tensor map (x, y, z, component) over the padded field copy; the step kernel
+// fetches a supercell's whole E/B tile with one cp.async.bulk.tensor.
+// cuTensorMapEncodeTiled is resolved through the runtime, so libcuda is not a link dependency.
+static int pic_build_tensor_map(pic_ctx* c)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+    if (e != cudaSuccess || !fn || qres != cudaDriverEntryPointSuccess) {
+        cudaGetLastError();
+        return fail(c, PIC_ECUDA, "cuTensorMapEncodeTiled not available");
+    }
+    const PicDev& d = c->d;
+    const int O = c->order;
+    const cuuint32_t fn_xy = (O == 1) ? 10 : (O == 2) ? 11 : 12;
+    const cuuint64_t px = d.nx + PIC_PAD_X, py = d.ny + PIC_PAD_Y, pz = d.nz + PIC_PAD_Z;
+    const cuuint64_t dims[4] = {px, py, pz, 6};
+    const cuuint64_t strides[3] = {px * 4, px * py * 4, px * py * pz * 4};
+    const cuuint32_t box[4] = {12, fn_xy, fn_xy - (PIC_SCX - PIC_SCZ), 6};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult r = ((encode_fn)fn)((CUtensorMap*)c->tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void*)d.Fpad, dims,
+                                 strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                 CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(c, PIC_ECUDA, "cuTensorMapEncodeTiled failed");
+    return PIC_OK;
+}
+
+// ------------------------------------------------------------------ C ABI
+extern "C" {
+
+int32_t pic_workspace_bytes(const int32_t grid[3], const int32_t supercell[3], int32_t shape_order,
+                            int64_t max_particles, uint64_t* bytes_out)
+{
+    Layout L;
+    int rc = compute_layout(grid, supercell, shape_order, max_particles, &L);
+    if (rc != PIC_OK) return fail(nullptr, rc, "pic_workspace_bytes: bad geometry (grid must be a positive multiple of the 8x8x4 supercell, order in 1..3)");
+    if (!bytes_out) return fail(nullptr, PIC_EINVAL, "pic_workspace_bytes: bytes_out is NULL");
+    *bytes_out = L.total;
+    return PIC_OK;
+}
+
+int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], double dt,
+                   const int32_t supercell[3], int32_t shape_order, int64_t max_particles,
+                   void* workspace, uint64_t workspace_bytes, void* stream)
+{
+    if (!out) return fail(nullptr, PIC_EINVAL, "pic_create: out is NULL");
+    *out = nullptr;
+    Layout L;
+    int rc = compute_layout(grid, supercell, shape_order, max_particles, &L);
+    if (rc != PIC_OK) return fail(nullptr, rc, "pic_create: bad geometry (grid must be a positive multiple of the 8x8x4 supercell, order in 1..3)");
+    if (!cell || !(dt > 0.0)) return fail(nullptr, PIC_EINVAL, "pic_create: cell is NULL or dt <= 0");
+    for (int a = 0; a < 3; ++a)
+        if (!(cell[a] > 0.0) || !(dt < cell[a]))
+            return fail(nullptr, PIC_EINVAL, "pic_create: need cell > 0 and c*dt < cell on every axis");
+    if (!workspace || ((uintptr_t)workspace & 255)) return fail(nullptr, PIC_EINVAL, "pic_create: workspace is NULL or not 256-byte aligned");
+    if (workspace_bytes < L.total) return fail(nullptr, PIC_ENOMEM, "pic_create: workspace smaller than pic_workspace_bytes()");
+
+    pic_ctx* c = new (std::nothrow) pic_ctx();
+    if (!c) return fail(nullptr, PIC_ENOMEM, "pic_create: host allocation failed");
+    c->order = shape_order;
+    c->dt = dt;
+    for (int a = 0; a < 3; ++a) c->cell[a] = cell[a];
+    for (int s = 0; s < PIC_NSPECIES; ++s) { c->q[s] = -1.0; c->m[s] = 1.0; }
+    c->max_particles = max_particles;
+    c->n_particles = 0;
+    c->steps = 0;
+    c->launches = 0;
+    c->stream = (cudaStream_t)stream;
+    c->have_fields = false;
+    c->use_tma = true;
+    c->use_graph = false;
+    c->tmap_ok = false;
+    c->graph_exec = nullptr;
+    c->graph_steps = 0;
+    c->ws = (char*)workspace;
+    c->ws_bytes = workspace_bytes;
+
+    PicDev& d = c->d;
+    d.nx = grid[0]; d.ny = grid[1]; d.nz = grid[2];
+    d.nsx = grid[0] / PIC_SCX; d.nsy = grid[1] / PIC_SCY; d.nsz = grid[2] / PIC_SCZ;
+    d.nsc = L.nsc;
+    d.dtdx = (float)(dt / cell[0]); d.dtdy = (float)(dt / cell[1]); d.dtdz = (float)(dt / cell[2]);
+    const double V = cell[0] * cell[1] * cell[2];
+    d.jfx = (float)(cell[0] / dt / V); d.jfy = (float)(cell[1] / dt / V); d.jfz = (float)(cell[2] / dt / V);
+    refresh_species(c);
+    char* w = c->ws;
+    d.pos = (float4*)(w + L.pos); d.mom = (float4*)(w + L.mom); d.pid = (uint32_t*)(w + L.pid);
+    d.n_frames = L.n_frames;
+    d.tbl_pool = (int*)(w + L.tbl_pool); d.tbl_pool_size = L.tbl_pool_size;
+    d.tbl_off = (int*)(w + L.tbl_off); d.tbl_cap = (int*)(w + L.tbl_cap);
+    d.sc_nframes = (int*)(w + L.sc_nframes); d.sc_count = (int*)(w + L.sc_count);
+    d.sc_stay = (int*)(w + L.sc_stay); d.sc_incoming = (int*)(w + L.sc_incoming);
+    d.x_pos = (float4*)(w + L.x_pos); d.x_mom = (float4*)(w + L.x_mom);
+    d.x_id = (uint32_t*)(w + L.x_id); d.x_dst = (int*)(w + L.x_dst); d.x_cap = L.x_cap;
+    d.ctr = (int*)(w + L.ctr); d.ctr64 = (unsigned long long*)(w + L.ctr64);
+    d.F = (const float*)(w + L.F); d.Fpad = (const float*)(w + L.Fpad); d.J = (float*)(w + L.J);
+    d.sc_offset = (long long*)(w + L.sc_offset);
+
+    // zero the bookkeeping region [tbl_off, x_pos) and the counters, J
+    cudaError_t e = cudaMemsetAsync(w + L.tbl_off, 0, L.x_pos - L.tbl_off, c->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(w + L.ctr, 0, L.F - L.ctr, c->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(w + L.J, 0, L.sc_offset - L.J, c->stream);
+    if (e != cudaSuccess) { int r = cuda_fail(nullptr, e, "pic_create: cudaMemsetAsync"); delete c; return r; }
+    *out = c;
+    return PIC_OK;
+}
+
+int32_t pic_set_species(pic_ctx* c, int32_t n, const double* q, const double* m)
+{
+    if (!c) return PIC_EINVAL;
+    if (n < 0 || n > PIC_MAX_SPECIES || !q || !m) return fail(c, PIC_EINVAL, "pic_set_species: n out of range or NULL table");
+    for (int s = 0; s < n; ++s) {
+        if (!(m[s] > 0.0)) return fail(c, PIC_EINVAL, "pic_set_species: mass must be positive");
+        c->q[s] = q[s]; c->m[s] = m[s];
+    }
+    refresh_species(c);
+    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    return PIC_OK;
+}
+
+int32_t pic_load_particles(pic_ctx* c, int64_t n, const double* x, const double* y, const double* z,
+                           const float* ux, const float* uy, const float* uz, const float* w,
+                           const int32_t* species)
+{
+    if (!c) return PIC_EINVAL;
+    if (n < 0) return fail(c, PIC_EINVAL, "pic_load_particles: n < 0");
+    if (n == 0) return PIC_OK;
+    if (!x || !y || !z || !ux || !uy || !uz || !w) return fail(c, PIC_EINVAL, "pic_load_particles: NULL array");
+    if (c->n_particles + n > c->max_particles) return fail(c, PIC_ENOMEM, "pic_load_particles: exceeds max_particles");
+    LoadArgs a;
+    a.x = x; a.y = y; a.z = z; a.ux = ux; a.uy = uy; a.uz = uz; a.w = w; a.species = species;
+    a.n = n; a.id0 = (unsigned)c->n_particles;
+    a.icx = 1.0 / c->cell[0]; a.icy = 1.0 / c->cell[1]; a.icz = 1.0 / c->cell[2];
+    const PicDev& d = c->d;
+    const int grid = (int)((n + 255) / 256 < 148 * 16 ? (n + 255) / 256 : 148 * 16);
+    pic_load_count_kernel<<<grid, 256, 0, c->stream>>>(d, a);
+    pic_copy_int_kernel<<<(d.nsc + 255) / 256, 256, 0, c->stream>>>(d.sc_stay, d.sc_count, d.nsc);
+    c->launches += 2;
+    cudaError_t e = pic_launch_resort(d, c->stream, &c->launches, false);   // frame allocation only
+    if (e != cudaSuccess) return cuda_fail(c, e, "pic_load_particles: prepare");
+    pic_load_scatter_kernel<<<grid, 256, 0, c->stream>>>(d, a);
+    c->launches += 1;
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e, "pic_load_particles: scatter");
+    c->n_particles += n;
+    return PIC_OK;
+}
+
+int32_t pic_set_fields(pic_ctx* c, const float* Ex, const float* Ey, const float* Ez,
+                       const float* Bx, const float* By, const float* Bz)
+{
+    if (!c) return PIC_EINVAL;
+    const float* src[6] = {Ex, Ey, Ez, Bx, By, Bz};
+    const size_t ncell = (size_t)c->d.nx * c->d.ny * c->d.nz;
+    for (int k = 0; k < 6; ++k) {
+        if (!src[k]) return fail(c, PIC_EINVAL, "pic_set_fields: NULL component");
+        cudaError_t e = cudaMemcpyAsync((float*)c->d.F + k * ncell, src[k], ncell * sizeof(float),
+                                        cudaMemcpyDeviceToDevice, c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e, "pic_set_fields: cudaMemcpyAsync");
+    }
+    pic_pad_fields_kernel<<<148 * 8, 256, 0, c->stream>>>(c->d, (float*)c->d.Fpad);
+    c->launches += 1;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e, "pic_set_fields: pad kernel");
+    if (!c->tmap_ok) c->tmap_ok = (pic_build_tensor_map(c) == PIC_OK);
+    c->have_fields = true;
+    return PIC_OK;
+}
+
+static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
+{
+    const PicDev& d = c->d;
+    const size_t ncell = (size_t)d.nx * d.ny * d.nz;
+    for (int i = 0; i < n; ++i) {
+        cudaError_t e = cudaMemsetAsync(d.J, 0, 3 * ncell * sizeof(float), st);          // S16
+        if (e == cudaSuccess) e = cudaMemsetAsync(d.ctr + CTR_EXCH, 0, sizeof(int), st);
+        if (e == cudaSuccess) e = pic_launch_step(d, c->order, c->use_tma && c->tmap_ok, c->tmap, st, &c->launches);
+        if (e == cudaSuccess) e = pic_launch_resort(d, st, &c->launches, true);
+        if (e != cudaSuccess) return cuda_fail(c, e, "pic_step: launch");
+    }
+    return PIC_OK;
+}
+
+int32_t pic_step(pic_ctx* c, int32_t n)
+{
+    if (!c) return PIC_EINVAL;
+    if (n < 0) return fail(c, PIC_EINVAL, "pic_step: n < 0");
+    if (!c->have_fields) return fail(c, PIC_ESTATE, "pic_step: pic_set_fields has not been called");
+    if (c->n_particles == 0) return fail(c, PIC_ESTATE, "pic_step: no particles loaded");
+    int rc = enqueue_steps(c, n, c->stream);
+    if (rc == PIC_OK) c->steps += n;
+    return rc;
+}
+
+int32_t pic_get_current(pic_ctx* c, float* Jx, float* Jy, float* Jz)
+{
+    if (!c) return PIC_EINVAL;
+    float* dst[3] = {Jx, Jy, Jz};
+    const size_t ncell = (size_t)c->d.nx * c->d.ny * c->d.nz;
+    for (int k = 0; k < 3; ++k) {
+        if (!dst[k]) continue;
+        cudaError_t e = cudaMemcpyAsync(dst[k], c->d.J + k * ncell, ncell * sizeof(float),
+                                        cudaMemcpyDeviceToDevice, c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e, "pic_get_current: cudaMemcpyAsync");
+    }
+    return PIC_OK;
+}
+
+int32_t pic_get_particles(pic_ctx* c, int64_t capacity, int64_t* n_out, double* x, double* y, double* z,
+                          float* ux, float* uy, float* uz, float* w, int32_t* species, uint32_t* id,
+                          int32_t* supercell)
+{
+    if (!c) return PIC_EINVAL;
+    if (capacity < 0) return fail(c, PIC_EINVAL, "pic_get_particles: capacity < 0");
+    const PicDev& d = c->d;
+    pic_scan_counts_kernel<<<1, 1024, 0, c->stream>>>(d);
+    GetArgs a;
+    a.x = x; a.y = y; a.z = z; a.ux = ux; a.uy = uy; a.uz = uz; a.w = w;
+    a.species = species; a.id = id; a.supercell = supercell; a.capacity = capacity;
+    a.cx = c->cell[0]; a.cy = c->cell[1]; a.cz = c->cell[2];
+    pic_get_particles_kernel<<<d.nsc, 256, 0, c->stream>>>(d, a);
+    c->launches += 2;
+    long long total = 0;
+    cudaError_t e = cudaMemcpyAsync(&total, d.sc_offset + d.nsc, sizeof(long long), cudaMemcpyDeviceToHost, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "pic_get_particles: cudaMemcpyAsync");
+    int rc = check_device(c);   // synchronises
+    if (n_out) *n_out = total;
+    if (rc != PIC_OK) return rc;
+    if (total > capacity) return fail(c, PIC_ENOMEM, "pic_get_particles: capacity smaller than the particle count");
+    return PIC_OK;
+}
+
+int32_t pic_get_counts(pic_ctx* c, int32_t* per_supercell_count)
+{
+    if (!c) return PIC_EINVAL;
+    if (!per_supercell_count) return fail(c, PIC_EINVAL, "pic_get_counts: NULL");
+    cudaError_t e = cudaMemcpyAsync(per_supercell_count, c->d.sc_count, (size_t)c->d.nsc * sizeof(int),
+                                    cudaMemcpyDeviceToDevice, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "pic_get_counts: cudaMemcpyAsync");
+    return PIC_OK;
+}
+
+int32_t pic_get_stats(pic_ctx* c, int64_t stats[8])
+{
+    if (!c) return PIC_EINVAL;
+    if (!stats) return fail(c, PIC_EINVAL, "pic_get_stats: NULL");
+    int ctr[CTR_N];
+    unsigned long long c64[CTR64_N];
+    cudaError_t e = cudaMemcpyAsync(ctr, c->d.ctr, sizeof ctr, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c64, c->d.ctr64, sizeof c64, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "pic_get_stats");
+    stats[0] = c->n_particles;
+    stats[1] = ctr[CTR_LEAVERS_LAST];
+    stats[2] = ctr[CTR_POOL_TOP];
+    stats[3] = c->d.n_frames;
+    stats[4] = ctr[CTR_MAX_COUNT];
+    stats[5] = c->steps;
+    stats[6] = (int64_t)c64[CTR64_LEAVERS_CUM];
+    stats[7] = ctr[CTR_ERROR];
+    if (ctr[CTR_ERROR]) return fail(c, PIC_EDEVICE, "pic_get_stats: sticky device fault, see stats[7]");
+    return PIC_OK;
+}
+
+int32_t pic_sync(pic_ctx* c)
+{
+    if (!c) return PIC_EINVAL;
+    return check_device(c);
+}
+
+int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
+{
+    if (!c || !key) return PIC_EINVAL;
+    if (!strcmp(key, "tma")) { c->use_tma = value != 0; return PIC_OK; }
+    if (!strcmp(key, "graph")) { c->use_graph = value != 0; return PIC_OK; }
+    return fail(c, PIC_EINVAL, std::string("pic_set_option: unknown key ") + key);
+}
+
+int64_t pic_launch_count(const pic_ctx* c) { return c ? c->launches : 0; }
+
+const char* pic_last_error(const pic_ctx* c) { return c ? c->err.c_str() : g_create_error.c_str(); }
+
+int32_t pic_destroy(pic_ctx* c)
+{
+    if (!c) return PIC_EINVAL;
+    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    delete c;
+    return PIC_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,149 @@
+"""CUDA-vs-oracle parity of the PIC particle step, through the C ABI (binding.Pic).
+
+Cases: configs[0] at full size (1 and 10 steps) and reduced-grid copies of configs[1..4]
+(same ppc, shape order, field recipe; SURVEY.md §8(d) tier T2), each spanning several
+supercells, several frames per supercell and a ragged last frame.  Tolerances: tests/pic_parity.py.
+"""
+import numpy as np
+import pytest
+import torch
+
+import pic_parity as PP
+from paper_2110_08650_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+CASES = {
+    # name: (workload, u_scale for the momentum tolerance (S17))
+    "cfg1_tiny_cic": (W.CONFIGS["tiny_thermal"], 0.01),
+    "cfg2_thermal_tsc_32": (W.CONFIGS["thermal_128"].scaled((32, 32, 32)), 0.05),
+    "cfg3_lwfa_tsc_32x128x32": (W.CONFIGS["lwfa"].scaled((32, 128, 32)), 1e-3),
+    "cfg4_khi_tsc_24": (W.CONFIGS["khi"].scaled((24, 24, 24)), 0.01),
+    "cfg4_khi_hotspot_tsc_24": (W.CONFIGS["khi_hotspot"].scaled((24, 24, 24)), 0.01),
+    "cfg5_pqs_32x32x16": (W.CONFIGS["pqs_large"].scaled((32, 32, 16)), 0.1),
+}
+
+
+def _run(name, n_steps, **options):
+    wl, u_scale = CASES[name]
+    parts, fields = W.make_particles(wl), W.make_fields(wl)
+    orc = PP.oracle_for(wl, parts, fields)
+    pic = PP.gpu_for(wl, parts, fields, **options)
+    assert orc.step(n_steps) == 0
+    pic.step(n_steps)
+    pic.sync()
+    rep = PP.compare(wl, orc, pic, n_steps, u_scale)
+    print(f"\n[{name} steps={n_steps} {options}] {rep}")
+    st = pic.get_stats()
+    assert st["error"] == 0 and st["particles"] == parts.n and st["steps"] == n_steps
+    assert PP.gpu_membership_consistent(wl, pic)
+    return rep, pic, wl
+
+
+@pytest.mark.parametrize("name", list(CASES))
+@pytest.mark.parametrize("tma", (0, 1))
+def test_one_step(name, tma):
+    rep, pic, wl = _run(name, 1, tma=tma)
+    assert rep.max_dx <= PP.TOL_X
+    assert rep.max_du_rel <= PP.TOL_U
+    assert rep.j_err_rel <= PP.TOL_J1
+    assert rep.n_member_mismatch == 0 and rep.counts_equal_outside_band
+    pic.destroy()
+
+
+@pytest.mark.parametrize("name", ["cfg1_tiny_cic", "cfg2_thermal_tsc_32", "cfg4_khi_hotspot_tsc_24", "cfg5_pqs_32x32x16"])
+def test_ten_steps_free_running(name):
+    rep, pic, wl = _run(name, 10)
+    assert rep.max_dx <= 10 * PP.TOL_X
+    assert rep.max_du_rel <= 10 * PP.TOL_U
+    assert rep.j_err_rel <= PP.TOL_J10
+    assert rep.n_member_mismatch == 0 and rep.counts_equal_outside_band
+    pic.destroy()
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_gpu_continuity(name):
+    """The GPU's own J and positions satisfy the discrete continuity equation (S22)."""
+    wl, _ = CASES[name]
+    parts, fields = W.make_particles(wl), W.make_fields(wl)
+    pic = PP.gpu_for(wl, parts, fields)
+    pic.step(2)     # not from the pristine state: resorted frames, arrivals appended
+    res = PP.gpu_continuity(wl, pic, [-1.0] * 16)
+    print(f"\n[{name}] continuity residual {res:.3e}")
+    assert res <= PP.TOL_CONT
+    pic.destroy()
+
+
+def test_species_table_and_anisotropic_cells():
+    """Positive charge / heavier species and dx != dy != dz go through the same kernels."""
+    wl = W.CONFIGS["khi"].scaled((16, 24, 8), cell=(1.0, 0.8, 1.25), dt=0.4)
+    parts, fields = W.make_particles(wl), W.make_fields(wl)
+    orc = PP.oracle_for(wl, parts, fields)
+    orc.set_species([-1.0, 2.0], [1.0, 4.0])
+    pic = PP.gpu_for(wl, parts, fields)
+    pic.set_species([-1.0, 2.0], [1.0, 4.0])
+    assert orc.step(3) == 0
+    pic.step(3)
+    rep = PP.compare(wl, orc, pic, 3, 0.01)
+    print(f"\n[species/anisotropic] {rep}")
+    assert rep.max_dx <= 3 * PP.TOL_X and rep.max_du_rel <= 3 * PP.TOL_U and rep.j_err_rel <= 3 * PP.TOL_J1
+    assert rep.n_member_mismatch == 0
+    pic.destroy()
+
+
+def test_append_loads_and_empty_supercells():
+    """Repeated pic_load_particles calls append; supercells without particles are fine."""
+    wl = W.CONFIGS["lwfa"].scaled((16, 64, 8))
+    fields = W.make_fields(wl)
+    chunks = list(W.particle_chunks(wl, max_chunk=2048))
+    assert len(chunks) > 2
+    parts = W.ParticleChunk.cat(chunks)
+    orc = PP.oracle_for(wl, parts, fields)
+    from paper_2110_08650_b200.binding import Pic
+    pic = Pic(wl.grid, wl.cell, wl.dt, wl.supercell, wl.shape_order, max_particles=parts.n)
+    for c in chunks:
+        g = c.to("cuda:0")
+        pic.load_particles(g.x, g.y, g.z, g.ux, g.uy, g.uz, g.w, g.species)
+        pic.sync()
+    pic.set_fields(fields.cuda())
+    counts0 = pic.get_counts().cpu().numpy()
+    assert counts0.sum() == parts.n and (counts0 == 0).any()
+    assert orc.step(2) == 0
+    pic.step(2)
+    rep = PP.compare(wl, orc, pic, 2, 1e-3)
+    print(f"\n[append] {rep}")
+    assert rep.max_dx <= 2 * PP.TOL_X and rep.max_du_rel <= 2 * PP.TOL_U and rep.j_err_rel <= 2 * PP.TOL_J1
+    assert rep.n_member_mismatch == 0
+    pic.destroy()
+
+
+def test_roundtrip_without_step():
+    """load -> get returns the same multiset, exactly (positions are integer + fp32 fraction)."""
+    wl = W.CONFIGS["thermal_128"].scaled((16, 16, 8), ppc=5)
+    parts = W.make_particles(wl)
+    pic = PP.gpu_for(wl, parts, W.make_fields(wl))
+    G = PP.gpu_particles_by_id(pic)
+    for k in ("x", "y", "z", "ux", "uy", "uz", "w", "species"):
+        assert np.array_equal(G[k], getattr(parts, k).numpy()), k
+    assert PP.gpu_membership_consistent(wl, pic)
+    pic.destroy()
+
+
+def test_error_paths():
+    from paper_2110_08650_b200.binding import Pic, PicError, PIC_EINVAL, PIC_ESTATE, PIC_ENOMEM
+    with pytest.raises(PicError) as e:
+        Pic((20, 16, 16), max_particles=10)            # not a multiple of the supercell
+    assert e.value.code == PIC_EINVAL
+    with pytest.raises(PicError) as e:
+        Pic((16, 16, 16), dt=1.5, max_particles=10)    # c*dt >= cell
+    assert e.value.code == PIC_EINVAL
+    pic = Pic((16, 16, 16), max_particles=4)
+    with pytest.raises(PicError) as e:
+        pic.step(1)                                    # no fields yet
+    assert e.value.code == PIC_ESTATE
+    z64 = torch.zeros(8, dtype=torch.float64, device="cuda")
+    z32 = torch.zeros(8, dtype=torch.float32, device="cuda")
+    with pytest.raises(PicError) as e:
+        pic.load_particles(z64, z64, z64, z32, z32, z32, z32)   # over capacity
+    assert e.value.code == PIC_ENOMEM
+    pic.destroy()
