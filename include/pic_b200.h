@@ -18,8 +18,8 @@
  * (pic_workspace_bytes() -> size; allocate it e.g. as a torch uint8 tensor, 256-byte
  * aligned; hand it to pic_create; free it after pic_destroy).  All work is enqueued
  * on the cudaStream_t given to pic_create; calls that return host values
- * (pic_get_particles' n_out, pic_get_counts to a host buffer is NOT offered —
- * see each call) synchronise that stream, the others are asynchronous.
+ * (pic_get_particles, pic_get_stats, pic_get_timing, pic_sync) synchronise that
+ * stream, the others are asynchronous.
  *
  * Array layout.  Grid arrays (E, B, J components) are float32 of nx*ny*nz elements,
  * index i + nx*(j + ny*k), each component sampled at its Yee location
@@ -133,10 +133,16 @@ int32_t pic_get_stats(pic_ctx* ctx, int64_t stats[8]);
 /* Wait for the stream and report a sticky device error, if any. */
 int32_t pic_sync(pic_ctx* ctx);
 
-/* Kernel variant switches for measurement (all variants compute the same step):
- * key "tma" (1 = stage E/B tiles with cp.async.bulk.tensor, 0 = plain loads),
- * key "graph" (1 = replay pic_step through a CUDA graph).  Host strings. */
+/* Kernel variant / measurement switches (all variants compute the same step):
+ * key "tma" (1 = stage E/B tiles with cp.async.bulk.tensor, 0 = plain loads; default 1),
+ * key "timing" (1 = record CUDA events around every launch of the step kernel, read
+ * with pic_get_timing; default 0).  key is a host string. */
 int32_t pic_set_option(pic_ctx* ctx, const char* key, int64_t value);
+
+/* With option "timing": total device time in ms of the step-kernel launches since the
+ * last call, and how many there were (host pointers, either may be NULL).  Synchronises
+ * and resets the accumulation. */
+int32_t pic_get_timing(pic_ctx* ctx, double* step_kernel_ms, int64_t* step_kernel_launches);
 
 /* Number of kernel launches enqueued by this context so far (host counter). */
 int64_t pic_launch_count(const pic_ctx* ctx);

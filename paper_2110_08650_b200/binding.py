@@ -22,7 +22,7 @@ _CODES = {0: "PIC_OK", -1: "PIC_EINVAL", -2: "PIC_ENOMEM", -3: "PIC_ECUDA", -4: 
 SYMBOLS = (
     "pic_workspace_bytes", "pic_create", "pic_set_species", "pic_load_particles", "pic_set_fields",
     "pic_step", "pic_get_current", "pic_get_particles", "pic_get_counts", "pic_get_stats", "pic_sync",
-    "pic_set_option", "pic_launch_count", "pic_last_error", "pic_destroy",
+    "pic_set_option", "pic_get_timing", "pic_launch_count", "pic_last_error", "pic_destroy",
 )
 
 
@@ -61,6 +61,7 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     L.pic_get_stats.argtypes = [vp, C.POINTER(i64)]
     L.pic_sync.argtypes = [vp]
     L.pic_set_option.argtypes = [vp, C.c_char_p, i64]
+    L.pic_get_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(i64)]
     L.pic_launch_count.argtypes = [vp]
     L.pic_launch_count.restype = i64
     L.pic_last_error.argtypes = [vp]
@@ -101,7 +102,8 @@ class Pic:
     """One simulation context.  Method names mirror the C ABI without the ``pic_`` prefix."""
 
     def __init__(self, grid, cell=(1.0, 1.0, 1.0), dt=0.5, supercell=(8, 8, 4), shape_order=1,
-                 max_particles=0, device="cuda:0", stream: Optional[torch.cuda.Stream] = None):
+                 max_particles=0, device="cuda:0", stream: Optional[torch.cuda.Stream] = None,
+                 workspace: Optional[torch.Tensor] = None):
         self._L = load_library()
         self._h = C.c_void_p(None)
         if not torch.cuda.is_available():
@@ -119,7 +121,12 @@ class Pic:
         nbytes = workspace_bytes(self.grid, self.supercell, self.shape_order, self.max_particles)
         with torch.cuda.device(self.device):
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            if workspace is not None:
+                if not workspace.is_cuda or workspace.dtype != torch.uint8 or workspace.numel() < nbytes + 256:
+                    raise ValueError("workspace must be a CUDA uint8 tensor of >= workspace_bytes()+256 elements")
+                self.workspace = workspace
+            else:
+                self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
         base = self.workspace.data_ptr()
         aligned = (base + 255) // 256 * 256
         h = C.c_void_p(None)
@@ -204,6 +211,12 @@ class Pic:
 
     def set_option(self, key: str, value: int):
         self._check(self._L.pic_set_option(self._h, key.encode(), int(value)))
+
+    def get_timing(self) -> Tuple[float, int]:
+        """(total ms of step-kernel launches since the last call, number of launches); needs option timing=1."""
+        ms, n = C.c_double(0.0), C.c_int64(0)
+        self._check(self._L.pic_get_timing(self._h, C.byref(ms), C.byref(n)))
+        return float(ms.value), int(n.value)
 
     def launch_count(self) -> int:
         return int(self._L.pic_launch_count(self._h))

@@ -8,6 +8,7 @@
 
 #include <new>
 #include <string>
+#include <vector>
 
 #include "../../include/pic_b200.h"
 #include "pic_internal.cuh"
@@ -29,6 +30,9 @@ struct pic_ctx {
     bool tmap_ok;
     cudaGraphExec_t graph_exec;
     int graph_steps;
+    // option "timing": CUDA events around every launch of the step kernel
+    bool timing;
+    std::vector<cudaEvent_t> events;
 };
 
 static std::string g_create_error;
@@ -248,7 +252,7 @@ __global__ void pic_pad_fields_kernel(const PicDev d, float* dst)
         int j = (int)(r % py); r /= py;
         int k = (int)(r % pz);
         int c = (int)(r / pz);
-        int gi = ((i - PIC_PAD_LO) % d.nx + d.nx) % d.nx;
+        int gi = ((i - d.pad_lo_x) % d.nx + d.nx) % d.nx;
         int gj = ((j - PIC_PAD_LO) % d.ny + d.ny) % d.ny;
         int gk = ((k - PIC_PAD_LO) % d.nz + d.nz) % d.nz;
         dst[e] = d.F[c * ncell + (size_t)gi + (size_t)d.nx * ((size_t)gj + (size_t)d.ny * gk)];
@@ -356,6 +360,7 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     c->tmap_ok = false;
     c->graph_exec = nullptr;
     c->graph_steps = 0;
+    c->timing = false;
     c->ws = (char*)workspace;
     c->ws_bytes = workspace_bytes;
 
@@ -379,6 +384,7 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     d.ctr = (int*)(w + L.ctr); d.ctr64 = (unsigned long long*)(w + L.ctr64);
     d.F = (const float*)(w + L.F); d.Fpad = (const float*)(w + L.Fpad); d.J = (float*)(w + L.J);
     d.sc_offset = (long long*)(w + L.sc_offset);
+    d.pad_lo_x = (shape_order == 3) ? 2 : 1;
 
     // zero the bookkeeping region [tbl_off, x_pos) and the counters, J
     cudaError_t e = cudaMemsetAsync(w + L.tbl_off, 0, L.x_pos - L.tbl_off, c->stream);
@@ -458,7 +464,18 @@ static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
     for (int i = 0; i < n; ++i) {
         cudaError_t e = cudaMemsetAsync(d.J, 0, 3 * ncell * sizeof(float), st);          // S16
         if (e == cudaSuccess) e = cudaMemsetAsync(d.ctr + CTR_EXCH, 0, sizeof(int), st);
+        cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+        if (e == cudaSuccess && c->timing) {
+            e = cudaEventCreate(&ev0);
+            if (e == cudaSuccess) e = cudaEventCreate(&ev1);
+            if (e == cudaSuccess) e = cudaEventRecord(ev0, st);
+        }
         if (e == cudaSuccess) e = pic_launch_step(d, c->order, c->use_tma && c->tmap_ok, c->tmap, st, &c->launches);
+        if (e == cudaSuccess && c->timing) {
+            e = cudaEventRecord(ev1, st);
+            c->events.push_back(ev0);
+            c->events.push_back(ev1);
+        }
         if (e == cudaSuccess) e = pic_launch_resort(d, st, &c->launches, true);
         if (e != cudaSuccess) return cuda_fail(c, e, "pic_step: launch");
     }
@@ -557,7 +574,27 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
     if (!c || !key) return PIC_EINVAL;
     if (!strcmp(key, "tma")) { c->use_tma = value != 0; return PIC_OK; }
     if (!strcmp(key, "graph")) { c->use_graph = value != 0; return PIC_OK; }
+    if (!strcmp(key, "timing")) { c->timing = value != 0; return PIC_OK; }
     return fail(c, PIC_EINVAL, std::string("pic_set_option: unknown key ") + key);
+}
+
+int32_t pic_get_timing(pic_ctx* c, double* step_kernel_ms, int64_t* step_kernel_launches)
+{
+    if (!c) return PIC_EINVAL;
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "pic_get_timing: synchronize");
+    double total = 0.0;
+    for (size_t i = 0; i + 1 < c->events.size(); i += 2) {
+        float ms = 0.f;
+        e = cudaEventElapsedTime(&ms, c->events[i], c->events[i + 1]);
+        if (e != cudaSuccess) return cuda_fail(c, e, "pic_get_timing: cudaEventElapsedTime");
+        total += ms;
+    }
+    if (step_kernel_ms) *step_kernel_ms = total;
+    if (step_kernel_launches) *step_kernel_launches = (int64_t)(c->events.size() / 2);
+    for (cudaEvent_t ev : c->events) cudaEventDestroy(ev);
+    c->events.clear();
+    return PIC_OK;
 }
 
 int64_t pic_launch_count(const pic_ctx* c) { return c ? c->launches : 0; }
@@ -568,6 +605,7 @@ int32_t pic_destroy(pic_ctx* c)
 {
     if (!c) return PIC_EINVAL;
     if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    for (cudaEvent_t ev : c->events) cudaEventDestroy(ev);
     delete c;
     return PIC_OK;
 }

@@ -65,6 +65,8 @@ struct PicDev {
     // grids
     const float* F;              // 6 components x ncell (Ex,Ey,Ez,Bx,By,Bz), unpadded
     const float* Fpad;           // padded copy for TMA: [6][nz+PZ][ny+PY][nx+PX]
+    int pad_lo_x;                // x halo below node 0 in Fpad = the tile's guard width, so that
+                                 // every TMA box starts on a 16-byte boundary
     float* J;                    // 3 components x ncell
     // scratch
     long long* sc_offset;        // [nsc+1] exclusive scan of sc_count (pic_get_particles)

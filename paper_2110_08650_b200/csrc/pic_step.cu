@@ -193,7 +193,7 @@ __global__ void __launch_bounds__(PIC_FRAME) pic_step_kernel(const PicDev d, con
             mbar_init(&s_bar, 1);
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             mbar_expect_tx(&s_bar, 6u * G::FCOMP * sizeof(float));
-            tma_load_4d(sF, &tmap, &s_bar, ox + PIC_PAD_LO - G::FL, oy + PIC_PAD_LO - G::FL,
+            tma_load_4d(sF, &tmap, &s_bar, ox /* pad_lo_x == FL: 16 B aligned */, oy + PIC_PAD_LO - G::FL,
                         oz + PIC_PAD_LO - G::FL, 0);
         }
         for (int e = tid; e < 3 * G::JCOMP; e += PIC_FRAME) sJ[e] = 0.0f;
