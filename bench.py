@@ -1,0 +1,319 @@
+#!/usr/bin/env python
+"""bench.py — particle-steps/s of the PIC particle step (gather + Boris + Esirkepov + resort).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+One "step" = one pass of the whole hot path (pic_step(1)) over all particles
+of the workload.  Default workload = BASELINE.json configs[1] (128^3 TSC thermal plasma, 16 ppc,
+33.5 M particles), the configuration the metric is quoted on.  Prints ONE JSON line (rank 0).
+
+N > 1: the path is single-GPU by contract (north_star); ranks run independent replicas of the
+workload ("replicas only"), no data-path collective; value = particles of all
+ranks * K / max-over-ranks device time.
+--impl reference: the fp64 single-threaded oracle timed on the host cores on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "particle-steps/s (gather+Boris+Esirkepov+resort)"
+UNIT = "particle-steps/s"
+PARTICLE_BYTES = 64.0      # float4 pos + float4 mom, read + write (SURVEY.md §8(d), 64 B basis)
+GRID_BYTES_PER_CELL = 36.0  # E+B read once (24 B) + J written once (12 B) per cell per step
+LEAVER_BYTES = 36.0 * 0.015
+
+
+def algorithmic_bytes_per_particle_step(wl, n_particles: int) -> float:
+    """B_alg = 64 + 36 * cells/particles + 0.54 (1.5 % leavers x 36 B)."""
+    return PARTICLE_BYTES + GRID_BYTES_PER_CELL * wl.n_cells / n_particles + LEAVER_BYTES
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ln in self.lines:
+            f = [v.strip() for v in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample_rate(wl, n_sample: int, n_steps: int = 1):
+    """Time the oracle (as it stands, single-threaded fp64) on the first n_sample particles of the
+    workload with the full-size fields.  Returns (particle-steps/s, seconds, n_sample)."""
+    import torch
+    import oracle
+    from paper_2110_08650_b200 import workloads as W
+    fields = W.make_fields(wl)
+    per_slab = wl.grid[0] * wl.grid[1] * wl.ppc
+    chunk = next(iter(W.particle_chunks(wl, max_chunk=max(n_sample, per_slab))))
+    sel = torch.randperm(chunk.n, generator=torch.Generator().manual_seed(7))[:n_sample]
+    orc = oracle.Oracle(wl.grid, wl.cell, wl.dt, wl.supercell, wl.shape_order)
+    orc.load_particles(*(getattr(chunk, k)[sel].numpy() for k in ("x", "y", "z", "ux", "uy", "uz", "w")),
+                       species=chunk.species[sel].numpy())
+    orc.set_fields(fields.numpy())
+    t0 = time.perf_counter()
+    rc = orc.step(n_steps)
+    dt = time.perf_counter() - t0
+    assert rc == 0
+    return orc.n * n_steps / dt, dt, orc.n
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores; each step = one oracle step
+    over a bounded sample of the workload (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2110_08650_b200 import workloads as W
+    wl = W.CONFIGS[args.workload]
+    n_sample = {1: 400_000, 2: 200_000, 3: 130_000}[wl.shape_order]
+    for _ in range(args.warmup):
+        oracle_sample_rate(wl, n_sample // 8)
+    t_tot, n_tot = 0.0, 0
+    for _ in range(args.steps):
+        _, dt, n = oracle_sample_rate(wl, n_sample)
+        t_tot += dt
+        n_tot += n
+    value = n_tot / t_tot
+    sample = f"{n_sample} particles of {wl.name} per step (random subset of the first z-slabs), full-size fields"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wl.name, "grid": list(wl.grid), "shape_order": wl.shape_order, "ppc": wl.ppc,
+                   "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2110_08650_b200 import workloads as W
+    from paper_2110_08650_b200.binding import Pic, workspace_bytes
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device; the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    wl = W.CONFIGS[args.workload]
+    n = W.n_particles(wl)
+    K, Wm = args.steps, max(args.warmup, 3)
+    ws = torch.empty(workspace_bytes(wl.grid, wl.supercell, wl.shape_order, n) + 256, dtype=torch.uint8, device=dev)
+
+    def fresh(host_inputs=None):
+        pic = Pic(wl.grid, wl.cell, wl.dt, wl.supercell, wl.shape_order, max_particles=n, device=dev, workspace=ws)
+        pic.set_option("tma", args.tma)
+        return pic
+
+    # ---------------------------------------------------------------- device-resident throughput
+    pic = fresh()
+    fields = W.make_fields(wl, device=dev)
+    for chunk in W.particle_chunks(wl, device=dev, max_chunk=1 << 23):
+        pic.load_particles(chunk.x, chunk.y, chunk.z, chunk.ux, chunk.uy, chunk.uz, chunk.w, chunk.species)
+        pic.sync()
+    del chunk
+    pic.set_fields(fields)
+    pic.step(Wm)
+    pic.sync()
+    pic.set_option("timing", 1)
+    l0 = pic.launch_count()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    barrier()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(pic.stream)
+    pic.step(K)
+    ev1.record(pic.stream)
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    clocks = sampler.stop() if rank == 0 else None
+    kernel_ms, n_kernel = pic.get_timing()
+    launches = pic.launch_count() - l0
+    pic.set_option("timing", 0)
+    stats = pic.get_stats()
+    t = torch.tensor([ms, kernel_ms / max(n_kernel, 1)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max, kernel_ms_avg = float(t[0]), float(t[1])
+    value = world * n * K / (ms_max * 1e-3)
+    pic.destroy()
+
+    # ---------------------------------------------------------------- end to end with host buffers
+    e2e_steps = min(K, args.e2e_steps)
+    names = ("x", "y", "z", "ux", "uy", "uz", "w", "species")
+    host = {k: [] for k in names}
+    for chunk in W.particle_chunks(wl, device=dev, max_chunk=1 << 23):
+        for k in names:
+            host[k].append(getattr(chunk, k).cpu())
+    host = {k: torch.cat(v).pin_memory() for k, v in host.items()}
+    host_fields = fields.cpu().pin_memory()
+    dev_in = {k: torch.empty_like(v, device=dev) for k, v in host.items()}
+    dev_fields = torch.empty_like(fields)
+    out_keys = ("x", "y", "z", "ux", "uy", "uz")
+    host_out = {k: torch.empty(n, dtype=host[k].dtype).pin_memory() for k in out_keys}
+    host_J = torch.empty((3,) + tuple(fields.shape[1:]), dtype=torch.float32).pin_memory()
+    h2d = sum(v.numel() * v.element_size() for v in host.values()) + host_fields.numel() * 4
+    d2h = sum(v.numel() * v.element_size() for v in host_out.values()) + host_J.numel() * 4
+
+    def e2e_step():
+        p = fresh()
+        for k in names:
+            dev_in[k].copy_(host[k], non_blocking=True)
+        dev_fields.copy_(host_fields, non_blocking=True)
+        p.load_particles(*(dev_in[k] for k in names))
+        p.set_fields(dev_fields)
+        p.step(1)
+        host_J.copy_(p.get_current(), non_blocking=True)
+        P = p.get_particles(n)
+        for k in out_keys:
+            host_out[k].copy_(P[k], non_blocking=True)
+        torch.cuda.synchronize()
+        p.destroy()
+
+    e2e_step()                      # warm-up (page-locking, allocator)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_step()
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    te = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_value = world * n * e2e_steps / float(te[0])
+
+    if rank == 0:
+        peak, peak_src = measured_peaks()
+        b_alg = algorithmic_bytes_per_particle_step(wl, n)
+        achieved = b_alg * n / (kernel_ms_avg * 1e-3) / 1e9
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "step_kernel_traffic.json")
+        if os.path.exists(tpath):
+            with open(tpath) as f:
+                tj = json.load(f)
+            if tj.get("workload") == wl.name:
+                traffic = tj.get("dram_bytes_per_launch")
+        cpu = None
+        if world == 1 and not args.no_cpu_baseline:
+            n_s = {1: 4_000_000, 2: 2_400_000, 3: 1_600_000}[wl.shape_order]
+            v, dt, ns = oracle_sample_rate(wl, n_s)
+            cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+                   "sample": f"{ns} particles of {wl.name} x 1 step ({dt:.1f} s), full-size fields, single thread of "
+                             f"{len(os.sched_getaffinity(0))} available"}
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": wl.name, "grid": list(wl.grid), "shape_order": wl.shape_order, "ppc": wl.ppc,
+                       "particles_per_gpu": n, "supercell": list(wl.supercell), "dt": wl.dt,
+                       "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "l2": f"inputs larger than L2: {n * 72 / 1e6:.0f} MB of particle state per step vs 126 MB",
+                       "tma": args.tma, "leavers_per_step": stats["leavers_last"]},
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": traffic, "peak_source": peak_src, "kernel": "pic_step_kernel",
+                         "kernel_ms": kernel_ms_avg, "bytes_per_particle_step": b_alg,
+                         "frac_of_8000_GBps": achieved / 8000.0,
+                         "kernel_share_of_step": kernel_ms_avg / (ms_max / K)},
+            "cpu_baseline": cpu,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "steps": e2e_steps},
+            "gpu_launches": launches, "clocks": clocks,
+        }))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
+    ap.add_argument("--workload", default="thermal_128")
+    ap.add_argument("--tma", type=int, default=1)
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
