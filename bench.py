@@ -177,6 +177,7 @@ def run_ours(args):
     def fresh(host_inputs=None):
         pic = Pic(wl.grid, wl.cell, wl.dt, wl.supercell, wl.shape_order, max_particles=n, device=dev, workspace=ws)
         pic.set_option("tma", args.tma)
+        pic.set_option("deposit", args.deposit)
         return pic
 
     # ---------------------------------------------------------------- device-resident throughput
@@ -283,7 +284,8 @@ def run_ours(args):
                        "particles_per_gpu": n, "supercell": list(wl.supercell), "dt": wl.dt,
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": f"inputs larger than L2: {n * 72 / 1e6:.0f} MB of particle state per step vs 126 MB",
-                       "tma": args.tma, "leavers_per_step": stats["leavers_last"]},
+                       "tma": args.tma, "deposit": "fixed-point int32 pair" if args.deposit else "float atomics",
+                       "leavers_per_step": stats["leavers_last"]},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": traffic, "peak_source": peak_src, "kernel": "pic_step_kernel",
                          "kernel_ms": kernel_ms_avg, "bytes_per_particle_step": b_alg,
@@ -306,6 +308,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--workload", default="thermal_128")
     ap.add_argument("--tma", type=int, default=1)
+    ap.add_argument("--deposit", type=int, default=1, help="1 fixed-point integer atomics, 0 float CAS atomics")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -21,7 +21,7 @@ struct pic_ctx {
     int64_t max_particles, n_particles, steps, launches;
     cudaStream_t stream;
     bool have_fields;
-    bool use_tma, use_graph;
+    bool use_tma, use_graph, fixed_point;
     char* ws;
     uint64_t ws_bytes;
     std::string err;
@@ -42,7 +42,7 @@ namespace {
 
 struct Layout {
     uint64_t pos, mom, pid, tbl_pool, tbl_off, tbl_cap, sc_nframes, sc_count, sc_stay, sc_incoming,
-        x_pos, x_mom, x_id, x_dst, ctr, ctr64, F, Fpad, J, sc_offset, total;
+        x_pos, x_mom, x_id, x_dst, ctr, ctr64, F, Fpad, J, J64, sc_offset, total;
     int n_frames, tbl_pool_size, x_cap, nsc;
 };
 
@@ -86,6 +86,7 @@ int compute_layout(const int32_t grid[3], const int32_t sc[3], int order, int64_
     L->F = take(6 * ncell * 4);
     L->Fpad = take(6ull * (grid[0] + PIC_PAD_X) * (grid[1] + PIC_PAD_Y) * (grid[2] + PIC_PAD_Z) * 4);
     L->J = take(3 * ncell * 4);
+    L->J64 = take(3 * ncell * 8);
     L->sc_offset = take((nsc + 1) * 8);
     L->total = o;
     L->n_frames = (int)n_frames;
@@ -152,6 +153,7 @@ __global__ void pic_load_count_kernel(const PicDev d, const LoadArgs a)
         int lc;
         int s = load_locate(d, a, i, P, lc);
         atomicAdd(d.sc_incoming + s, 1);
+        atomicMax(d.ctr + CTR_WMAX_BITS, __float_as_int(fabsf(a.w[i])));
     }
 }
 
@@ -265,6 +267,9 @@ void refresh_species(pic_ctx* c)
         c->d.h[s] = (float)((c->q[s] / c->m[s]) * c->dt * 0.5);
         c->d.q[s] = (float)c->q[s];
     }
+    double qmax = 0.0;
+    for (int s = 0; s < PIC_NSPECIES; ++s) qmax = fmax(qmax, fabs(c->q[s]));
+    c->d.qmax = (float)qmax;
 }
 
 int check_device(pic_ctx* c)
@@ -357,6 +362,7 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     c->have_fields = false;
     c->use_tma = true;
     c->use_graph = false;
+    c->fixed_point = true;
     c->tmap_ok = false;
     c->graph_exec = nullptr;
     c->graph_steps = 0;
@@ -382,7 +388,7 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     d.x_pos = (float4*)(w + L.x_pos); d.x_mom = (float4*)(w + L.x_mom);
     d.x_id = (uint32_t*)(w + L.x_id); d.x_dst = (int*)(w + L.x_dst); d.x_cap = L.x_cap;
     d.ctr = (int*)(w + L.ctr); d.ctr64 = (unsigned long long*)(w + L.ctr64);
-    d.F = (const float*)(w + L.F); d.Fpad = (const float*)(w + L.Fpad); d.J = (float*)(w + L.J);
+    d.F = (const float*)(w + L.F); d.Fpad = (const float*)(w + L.Fpad); d.J = (float*)(w + L.J); d.J64 = (long long*)(w + L.J64);
     d.sc_offset = (long long*)(w + L.sc_offset);
     d.pad_lo_x = (shape_order == 3) ? 2 : 1;
 
@@ -462,7 +468,8 @@ static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
     const PicDev& d = c->d;
     const size_t ncell = (size_t)d.nx * d.ny * d.nz;
     for (int i = 0; i < n; ++i) {
-        cudaError_t e = cudaMemsetAsync(d.J, 0, 3 * ncell * sizeof(float), st);          // S16
+        cudaError_t e = c->fixed_point ? cudaMemsetAsync(d.J64, 0, 3 * ncell * sizeof(long long), st)   // S16
+                                       : cudaMemsetAsync(d.J, 0, 3 * ncell * sizeof(float), st);
         if (e == cudaSuccess) e = cudaMemsetAsync(d.ctr + CTR_EXCH, 0, sizeof(int), st);
         cudaEvent_t ev0 = nullptr, ev1 = nullptr;
         if (e == cudaSuccess && c->timing) {
@@ -470,7 +477,7 @@ static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
             if (e == cudaSuccess) e = cudaEventCreate(&ev1);
             if (e == cudaSuccess) e = cudaEventRecord(ev0, st);
         }
-        if (e == cudaSuccess) e = pic_launch_step(d, c->order, c->use_tma && c->tmap_ok, c->tmap, st, &c->launches);
+        if (e == cudaSuccess) e = pic_launch_step(d, c->order, c->use_tma && c->tmap_ok, c->fixed_point, c->tmap, st, &c->launches);
         if (e == cudaSuccess && c->timing) {
             e = cudaEventRecord(ev1, st);
             c->events.push_back(ev0);
@@ -574,6 +581,7 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
     if (!c || !key) return PIC_EINVAL;
     if (!strcmp(key, "tma")) { c->use_tma = value != 0; return PIC_OK; }
     if (!strcmp(key, "graph")) { c->use_graph = value != 0; return PIC_OK; }
+    if (!strcmp(key, "deposit")) { c->fixed_point = value != 0; return PIC_OK; }
     if (!strcmp(key, "timing")) { c->timing = value != 0; return PIC_OK; }
     return fail(c, PIC_EINVAL, std::string("pic_set_option: unknown key ") + key);
 }

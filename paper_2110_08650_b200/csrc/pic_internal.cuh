@@ -27,6 +27,7 @@ enum {
     CTR_ERROR = 3,        // sticky error word (PIC_DEV_* bits)
     CTR_LEAVERS_LAST = 4,
     CTR_MAX_COUNT = 5,
+    CTR_WMAX_BITS = 6,    // bits of max |weight| loaded so far (non-negative floats order like ints)
     CTR_N = 16
 };
 // 64-bit counters in PicDev::ctr64
@@ -40,6 +41,7 @@ struct PicDev {
     float jfx, jfy, jfz;         // (cell_a / dt) / (dx dy dz): J factor without q*w
     float h[PIC_NSPECIES];       // (q/m) dt / 2
     float q[PIC_NSPECIES];
+    float qmax;                  // max |q| over the species table
     // frames
     float4* pos;
     float4* mom;
@@ -68,6 +70,7 @@ struct PicDev {
     int pad_lo_x;                // x halo below node 0 in Fpad = the tile's guard width, so that
                                  // every TMA box starts on a 16-byte boundary
     float* J;                    // 3 components x ncell
+    long long* J64;              // fixed-point accumulators of the same shape (deposit option 1)
     // scratch
     long long* sc_offset;        // [nsc+1] exclusive scan of sc_count (pic_get_particles)
 };
@@ -84,6 +87,6 @@ __host__ __device__ inline uint32_t pic_pack_bits(int local_cell, int species)
 }
 
 // launchers implemented in pic_step.cu
-cudaError_t pic_launch_step(const PicDev& d, int order, bool use_tma, const void* tmap,
+cudaError_t pic_launch_step(const PicDev& d, int order, bool use_tma, bool fixed_point, const void* tmap,
                             cudaStream_t st, int64_t* launches);
 cudaError_t pic_launch_resort(const PicDev& d, cudaStream_t st, int64_t* launches, bool scatter);

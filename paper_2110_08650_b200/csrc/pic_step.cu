@@ -98,34 +98,6 @@ __device__ __forceinline__ void to_window(const float (&w)[O + 1], int off, floa
     }
 }
 
-// Esirkepov density decomposition of one component (SURVEY.md §8(c) step 6):
-// J_a[i,j,k] += fac * sum_{i'<=i} DS_a(i') * [S0_b S0_c + DS_b S0_c/2 + S0_b DS_c/2 + DS_b DS_c/3]
-// The tile pointer jt addresses the window's first node; strides sa, sb, sc follow
-// the flow axis a and the two transverse axes.
-template <int O>
-__device__ __forceinline__ void deposit1(float* jt, int sa, int sb, int sc, float fac,
-                                         const float (&DSa)[O + 2],
-                                         const float (&S0b)[O + 2], const float (&DSb)[O + 2],
-                                         const float (&S0c)[O + 2], const float (&DSc)[O + 2])
-{
-    constexpr int W = O + 2;
-#pragma unroll
-    for (int c = 0; c < W; ++c) {
-        const float c0 = S0c[c] + 0.5f * DSc[c];                 // multiplies S0b
-        const float c1 = 0.5f * S0c[c] + (1.0f / 3.0f) * DSc[c]; // multiplies DSb
-#pragma unroll
-        for (int b = 0; b < W; ++b) {
-            const float br = fac * fmaf(S0b[b], c0, DSb[b] * c1);
-            float acc = 0.0f;
-#pragma unroll
-            for (int a = 0; a < W - 1; ++a) {   // the last prefix is sum(DS) = 0: not written
-                acc = fmaf(DSa[a], br, acc);
-                if (acc != 0.0f) atomicAdd(jt + a * sa + b * sb + c * sc, acc);
-            }
-        }
-    }
-}
-
 __device__ __forceinline__ int wrapi(int i, int n)
 {
     if (i < 0) i += n;
@@ -167,25 +139,103 @@ __device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* map, u
         ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(x), "r"(y), "r"(z), "r"(c) : "memory");
 }
 
+// ------------------------------------------------------------------ fixed-point deposit
+// sm_100a has no native shared-memory float add (red.shared.add.f32 compiles to a
+// LDS + FADD + ATOMS.CAST.SPIN retry loop); 32-bit integer adds are native (ATOMS.ADD).
+// A contribution c (|c| <= cmax <= 2^e) is therefore split exactly into two integers on the
+// grid r = 2^(e-33):  c = (hi * 2^15 + lo) * r,  |hi| <= 2^18, |lo| <= 2^14, accumulated in two
+// int32 tiles.  Integer sums are associative, so the tile is bit-reproducible; a node overflows
+// only beyond 2^13 full-weight contributions (hi) or 2^17 contributions (lo).  DESIGN.md §deposit.
+#define PIC_FIX_MAGIC 12582912.0f          // 1.5 * 2^23: adding it rounds to an integer in the mantissa
+#define PIC_FIX_MAGIC_BITS 0x4B400000
+#define PIC_FIX_LO_BITS 15
+#define PIC_FIX_HI_LOG2 18
+
+// 2^(18-e) with |q|max * |w|max * jf <= 2^e: the same value in every CTA and in the convert kernel
+__device__ __forceinline__ float fix_scale_of(const PicDev& d, float jf)
+{
+    int e = 0;
+    frexpf(fmaxf(d.qmax * __int_as_float(d.ctr[CTR_WMAX_BITS]) * jf, 1e-30f), &e);
+    return ldexpf(1.0f, PIC_FIX_HI_LOG2 - e);
+}
+
+__device__ __forceinline__ void fix_add(int* hi, int* lo, int off, float v)
+{
+    const float t = v + PIC_FIX_MAGIC;                       // |v| <= 2^18: exact integer round(v)
+    const float rem = v - (t - PIC_FIX_MAGIC);               // exact, |rem| <= 1/2
+    const float t2 = fmaf(rem, (float)(1 << PIC_FIX_LO_BITS), PIC_FIX_MAGIC);
+    atomicAdd(hi + off, __float_as_int(t) - PIC_FIX_MAGIC_BITS);
+    atomicAdd(lo + off, __float_as_int(t2) - PIC_FIX_MAGIC_BITS);
+}
+
+// Esirkepov density decomposition of one component (SURVEY.md §8(c) step 6):
+// J_a[i,j,k] += fac * sum_{i'<=i} DS_a(i') * [S0_b S0_c + DS_b S0_c/2 + S0_b DS_c/2 + DS_b DS_c/3]
+// jt addresses the window's first node; strides sa, sb, sc follow the flow axis a and the
+// two transverse axes.  wa/wb/wc: warp-uniform "some lane uses the last window slot of this axis".
+template <int O, bool FIX>
+__device__ __forceinline__ void deposit1(float* jt, int* jhi, int* jlo, int base, int sa, int sb, int sc, float fac,
+                                         bool wa, bool wb, bool wc, bool lane_wa,
+                                         const float (&DSa)[O + 2],
+                                         const float (&S0b)[O + 2], const float (&DSb)[O + 2],
+                                         const float (&S0c)[O + 2], const float (&DSc)[O + 2])
+{
+    constexpr int W = O + 2;
+#pragma unroll
+    for (int c = 0; c < W; ++c) {
+        if (c == W - 1 && !wc) continue;
+        const float c0 = fac * (S0c[c] + 0.5f * DSc[c]);                 // multiplies S0b
+        const float c1 = fac * (0.5f * S0c[c] + (1.0f / 3.0f) * DSc[c]); // multiplies DSb
+#pragma unroll
+        for (int b = 0; b < W; ++b) {
+            if (b == W - 1 && !wb) continue;
+            const float br = fmaf(S0b[b], c0, DSb[b] * c1);
+            float acc = 0.0f;
+#pragma unroll
+            for (int a = 0; a < W - 1; ++a) {   // the last prefix is sum(DS) = 0: not written
+                if (a == W - 2 && !wa) continue;
+                acc = fmaf(DSa[a], br, acc);
+                // a lane whose own window is narrow has sum_{t<W-1} DS = 0 up to rounding: make it
+                // exactly 0, so that the result does not depend on which lanes share its warp
+                if (a == W - 2 && !lane_wa) acc = 0.0f;
+                const int off = base + a * sa + b * sb + c * sc;
+                if (FIX) {
+                    fix_add(jhi, jlo, off, acc);
+                } else {
+                    if (acc != 0.0f) atomicAdd(jt + off, acc);
+                }
+            }
+        }
+    }
+}
+
 // ------------------------------------------------------------------ the step kernel
-template <int O, bool TMA>
+template <int O, bool FIX> constexpr int step_smem_bytes()
+{
+    return (6 * Geo<O>::FCOMP + (FIX ? 6 : 3) * Geo<O>::JCOMP) * 4;
+}
+
+template <int O, bool TMA, bool FIX>
 __global__ void __launch_bounds__(PIC_FRAME) pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
 {
     using G = Geo<O>;
-    __shared__ __align__(128) float sF[6 * G::FCOMP];
-    __shared__ __align__(16) float sJ[3 * G::JCOMP];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float* sF = reinterpret_cast<float*>(smem_raw);                 // E/B tile [6][FNZ][FNY][FPX]
+    float* sJ = sF + 6 * G::FCOMP;                                  // float J tile [3][JNZ][JNY][JNX]
+    int* sJhi = reinterpret_cast<int*>(sJ);                         // or the fixed-point pair
+    int* sJlo = sJhi + 3 * G::JCOMP;
     __shared__ int s_wstay[PIC_FRAME / 32];
     __shared__ int s_wleave[PIC_FRAME / 32];
     __shared__ int s_xbase;
+    __shared__ __align__(8) uint64_t s_bar;
 
     const int tid = threadIdx.x;
     const int lane = tid & 31, warp = tid >> 5;
     const int s = blockIdx.x;
     const int ssx = s % d.nsx, ssy = (s / d.nsx) % d.nsy, ssz = s / (d.nsx * d.nsy);
     const int ox = ssx * PIC_SCX, oy = ssy * PIC_SCY, oz = ssz * PIC_SCZ;
+    constexpr int NJ = (FIX ? 6 : 3) * G::JCOMP;
 
     // ---- a2: stage the E/B tile and clear the J tile
-    __shared__ __align__(8) uint64_t s_bar;
     if (TMA) {
         // one bulk-tensor copy of the whole {12, FNY, FNZ, 6} box from the padded array
         // (periodic halos pre-filled by pic_set_fields); completion on an mbarrier
@@ -196,7 +246,7 @@ __global__ void __launch_bounds__(PIC_FRAME) pic_step_kernel(const PicDev d, con
             tma_load_4d(sF, &tmap, &s_bar, ox /* pad_lo_x == FL: 16 B aligned */, oy + PIC_PAD_LO - G::FL,
                         oz + PIC_PAD_LO - G::FL, 0);
         }
-        for (int e = tid; e < 3 * G::JCOMP; e += PIC_FRAME) sJ[e] = 0.0f;
+        for (int e = tid; e < NJ; e += PIC_FRAME) sJhi[e] = 0;
         __syncthreads();               // the barrier's init is visible to every waiter
         unsigned spins = 0;
         while (!mbar_try_wait(&s_bar, 0)) {
@@ -220,9 +270,17 @@ __global__ void __launch_bounds__(PIC_FRAME) pic_step_kernel(const PicDev d, con
             sF[c * G::FCOMP + (k * G::FNY + j) * G::FPX + i] =
                 __ldg(d.F + c * ncell + (size_t)gi + (size_t)d.nx * ((size_t)gj + (size_t)d.ny * gk));
         }
-        for (int e = tid; e < 3 * G::JCOMP; e += PIC_FRAME) sJ[e] = 0.0f;
+        for (int e = tid; e < NJ; e += PIC_FRAME) sJhi[e] = 0;
     }
     __syncthreads();
+
+    // fixed-point scale per component: 2^(18-e) with |q| wmax jf_a <= 2^e
+    float fix_scale[3] = {1.0f, 1.0f, 1.0f};
+    if (FIX) {
+        fix_scale[0] = fix_scale_of(d, d.jfx);
+        fix_scale[1] = fix_scale_of(d, d.jfy);
+        fix_scale[2] = fix_scale_of(d, d.jfz);
+    }
 
     const int count = d.sc_count[s];
     const int* tbl = d.tbl_pool + d.tbl_off[s];
@@ -232,15 +290,18 @@ __global__ void __launch_bounds__(PIC_FRAME) pic_step_kernel(const PicDev d, con
         const int slot = base + tid;
         const bool active = slot < count;
         bool stay = false;
-        float4 P = make_float4(0.f, 0.f, 0.f, 0.f), M = P;
-        uint32_t id = 0, bits = 0;
+        // lanes past the end of a partly filled warp are ghosts of zero weight
+        float4 P = make_float4(0.5f, 0.5f, 0.5f, 0.0f), M = make_float4(0.f, 0.f, 0.f, 0.f);
+        uint32_t id = 0;
         int dst = s;
-        if (active) {
-            const size_t idx = (size_t)tbl[slot >> 8] * PIC_FRAME + (slot & (PIC_FRAME - 1));
-            P = d.pos[idx];
-            M = d.mom[idx];
-            id = d.pid[idx];
-            bits = __float_as_uint(M.w);
+        if (base + warp * 32 < count) {        // warp-uniform: the warp holds at least one particle
+            if (active) {
+                const size_t idx = (size_t)tbl[slot >> 8] * PIC_FRAME + (slot & (PIC_FRAME - 1));
+                P = d.pos[idx];
+                M = d.mom[idx];
+                id = d.pid[idx];
+            }
+            const uint32_t bits = __float_as_uint(M.w);
             const int lc = bits & 0xffff, sp = (bits >> 16) & 0xff;
             const int cx = lc & 7, cy = (lc >> 3) & 7, cz = lc >> 6;
 
@@ -309,12 +370,15 @@ __global__ void __launch_bounds__(PIC_FRAME) pic_step_kernel(const PicDev d, con
             {
                 float S0[3][O + 2], DS[3][O + 2];
                 int lo[3];
+                bool wide[3], lwide[3];
 #pragma unroll
                 for (int a = 0; a < 3; ++a) {
                     float w0[O + 1], w1[O + 1], s1[O + 2];
                     int b0 = shape<O>(f0[a], w0);
                     int b1 = shape<O>(x1[a], w1);
                     lo[a] = min(b0, b1);
+                    lwide[a] = b0 != b1;                            // this lane uses the last window slot
+                    wide[a] = __any_sync(0xffffffffu, lwide[a]);    // ... some lane of the warp does
                     to_window<O>(w0, b0 - lo[a], S0[a]);
                     to_window<O>(w1, b1 - lo[a], s1);
 #pragma unroll
@@ -322,10 +386,13 @@ __global__ void __launch_bounds__(PIC_FRAME) pic_step_kernel(const PicDev d, con
                 }
                 const float qw = d.q[sp] * P.w;
                 constexpr int SX = 1, SY = G::JNX, SZ = G::JNX * G::JNY;
-                float* j0 = sJ + (cx + lo[0] + G::JL) * SX + (cy + lo[1] + G::JL) * SY + (cz + lo[2] + G::JL) * SZ;
-                deposit1<O>(j0 + 0 * G::JCOMP, SX, SY, SZ, -qw * d.jfx, DS[0], S0[1], DS[1], S0[2], DS[2]);
-                deposit1<O>(j0 + 1 * G::JCOMP, SY, SZ, SX, -qw * d.jfy, DS[1], S0[2], DS[2], S0[0], DS[0]);
-                deposit1<O>(j0 + 2 * G::JCOMP, SZ, SX, SY, -qw * d.jfz, DS[2], S0[0], DS[0], S0[1], DS[1]);
+                const int j0 = (cx + lo[0] + G::JL) * SX + (cy + lo[1] + G::JL) * SY + (cz + lo[2] + G::JL) * SZ;
+                deposit1<O, FIX>(sJ, sJhi, sJlo, j0 + 0 * G::JCOMP, SX, SY, SZ, -qw * d.jfx * fix_scale[0],
+                                 wide[0], wide[1], wide[2], lwide[0], DS[0], S0[1], DS[1], S0[2], DS[2]);
+                deposit1<O, FIX>(sJ, sJhi, sJlo, j0 + 1 * G::JCOMP, SY, SZ, SX, -qw * d.jfy * fix_scale[1],
+                                 wide[1], wide[2], wide[0], lwide[1], DS[1], S0[2], DS[2], S0[0], DS[0]);
+                deposit1<O, FIX>(sJ, sJhi, sJlo, j0 + 2 * G::JCOMP, SZ, SX, SY, -qw * d.jfz * fix_scale[2],
+                                 wide[2], wide[0], wide[1], lwide[2], DS[2], S0[0], DS[0], S0[1], DS[1]);
             }
 
             // ---- a5: new cell and destination supercell
@@ -334,8 +401,8 @@ __global__ void __launch_bounds__(PIC_FRAME) pic_step_kernel(const PicDev d, con
             int dsy = (ncy < 0) ? -1 : (ncy >= PIC_SCY) ? 1 : 0;
             int dsz = (ncz < 0) ? -1 : (ncz >= PIC_SCZ) ? 1 : 0;
             ncx -= dsx * PIC_SCX; ncy -= dsy * PIC_SCY; ncz -= dsz * PIC_SCZ;
-            stay = (dsx | dsy | dsz) == 0;
-            if (!stay)
+            stay = active && (dsx | dsy | dsz) == 0;
+            if (active && !stay)
                 dst = wrapi(ssx + dsx, d.nsx) + d.nsx * (wrapi(ssy + dsy, d.nsy) + d.nsy * wrapi(ssz + dsz, d.nsz));
             P.x = fn[0]; P.y = fn[1]; P.z = fn[2];
             M.w = __uint_as_float(pic_pack_bits(ncx + PIC_SCX * (ncy + PIC_SCY * ncz), sp));
@@ -390,19 +457,36 @@ __global__ void __launch_bounds__(PIC_FRAME) pic_step_kernel(const PicDev d, con
     {
         const size_t ncell = (size_t)d.nx * d.ny * d.nz;
         for (int e = tid; e < 3 * G::JCOMP; e += PIC_FRAME) {
-            const float v = sJ[e];
-            if (v != 0.0f) {
-                int i = e % G::JNX;
-                int r = e / G::JNX;
-                int j = r % G::JNY;
-                r /= G::JNY;
-                int k = r % G::JNZ;
-                int c = r / G::JNZ;
-                int gi = wrapi(ox + i - G::JL, d.nx), gj = wrapi(oy + j - G::JL, d.ny),
-                    gk = wrapi(oz + k - G::JL, d.nz);
-                atomicAdd(d.J + c * ncell + (size_t)gi + (size_t)d.nx * ((size_t)gj + (size_t)d.ny * gk), v);
+            int i = e % G::JNX;
+            int r = e / G::JNX;
+            int j = r % G::JNY;
+            r /= G::JNY;
+            int k = r % G::JNZ;
+            int c = r / G::JNZ;
+            int gi = wrapi(ox + i - G::JL, d.nx), gj = wrapi(oy + j - G::JL, d.ny),
+                gk = wrapi(oz + k - G::JL, d.nz);
+            const size_t g = c * ncell + (size_t)gi + (size_t)d.nx * ((size_t)gj + (size_t)d.ny * gk);
+            if (FIX) {
+                // 64-bit fixed point in global memory too (native RED.64 in L2): J is bit-reproducible
+                const long long n = ((long long)sJhi[e] << PIC_FIX_LO_BITS) + (long long)sJlo[e];
+                if (n != 0) atomicAdd(reinterpret_cast<unsigned long long*>(d.J64) + g, (unsigned long long)n);
+            } else {
+                const float v = sJ[e];
+                if (v != 0.0f) atomicAdd(d.J + g, v);
             }
         }
+    }
+}
+
+// Fixed-point global accumulators -> float J (one pass, after every CTA has flushed).
+__global__ void pic_convert_J_kernel(const PicDev d)
+{
+    const size_t ncell = (size_t)d.nx * d.ny * d.nz;
+    const float jf[3] = {d.jfx, d.jfy, d.jfz};
+    for (int c = 0; c < 3; ++c) {
+        const double inv = 1.0 / ((double)fix_scale_of(d, jf[c]) * (double)(1 << PIC_FIX_LO_BITS));
+        for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < ncell; i += (size_t)gridDim.x * blockDim.x)
+            d.J[c * ncell + i] = (float)((double)d.J64[c * ncell + i] * inv);
     }
 }
 
@@ -466,23 +550,44 @@ __global__ void pic_scatter_kernel(const PicDev d)
 
 }  // namespace
 
-cudaError_t pic_launch_step(const PicDev& d, int order, bool use_tma, const void* tmap,
+template <int O, bool TMA, bool FIX>
+static cudaError_t launch_step_variant(const PicDev& d, const CUtensorMap& map, cudaStream_t st)
+{
+    static bool configured = false;     // opt in to > 48 KB of dynamic shared memory once
+    constexpr int bytes = step_smem_bytes<O, FIX>();
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(pic_step_kernel<O, TMA, FIX>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    pic_step_kernel<O, TMA, FIX><<<d.nsc, PIC_FRAME, bytes, st>>>(d, map);
+    return cudaGetLastError();
+}
+
+cudaError_t pic_launch_step(const PicDev& d, int order, bool use_tma, bool fixed_point, const void* tmap,
                             cudaStream_t st, int64_t* launches)
 {
     CUtensorMap map;
     if (use_tma) memcpy(&map, tmap, sizeof map); else memset(&map, 0, sizeof map);
-#define PIC_GO(O, T) pic_step_kernel<O, T><<<d.nsc, PIC_FRAME, 0, st>>>(d, map)
-    switch (order * 2 + (use_tma ? 1 : 0)) {
-        case 2: PIC_GO(1, false); break;
-        case 3: PIC_GO(1, true); break;
-        case 4: PIC_GO(2, false); break;
-        case 5: PIC_GO(2, true); break;
-        case 6: PIC_GO(3, false); break;
-        default: PIC_GO(3, true); break;
+    cudaError_t e;
+#define PIC_GO(O)                                                                               \
+    e = use_tma ? (fixed_point ? launch_step_variant<O, true, true>(d, map, st)                 \
+                               : launch_step_variant<O, true, false>(d, map, st))               \
+                : (fixed_point ? launch_step_variant<O, false, true>(d, map, st)                \
+                               : launch_step_variant<O, false, false>(d, map, st))
+    switch (order) {
+        case 1: PIC_GO(1); break;
+        case 2: PIC_GO(2); break;
+        default: PIC_GO(3); break;
     }
 #undef PIC_GO
     ++*launches;
-    return cudaGetLastError();
+    if (e == cudaSuccess && fixed_point) {
+        pic_convert_J_kernel<<<148 * 8, 256, 0, st>>>(d);
+        ++*launches;
+        e = cudaGetLastError();
+    }
+    return e;
 }
 
 cudaError_t pic_launch_resort(const PicDev& d, cudaStream_t st, int64_t* launches, bool scatter)

@@ -52,6 +52,32 @@ def test_one_step(name, tma):
     pic.destroy()
 
 
+@pytest.mark.parametrize("name", ["cfg1_tiny_cic", "cfg2_thermal_tsc_32", "cfg5_pqs_32x32x16"])
+def test_float_atomic_deposit_variant(name):
+    """Option deposit=0 (float atomics on the shared J tile) computes the same step."""
+    rep, pic, wl = _run(name, 1, deposit=0)
+    assert rep.max_dx <= PP.TOL_X and rep.max_du_rel <= PP.TOL_U and rep.j_err_rel <= PP.TOL_J1
+    assert rep.n_member_mismatch == 0 and rep.counts_equal_outside_band
+    pic.destroy()
+
+
+def test_fixed_point_tile_is_order_independent():
+    """Fixed-point accumulation (shared tile and global J) is exact integer arithmetic: two runs whose
+    particles are loaded in different orders (different thread assignment and atomic order) give
+    bit-identical J."""
+    wl, _ = CASES["cfg2_thermal_tsc_32"]
+    parts, fields = W.make_particles(wl), W.make_fields(wl)
+    perm = torch.randperm(parts.n, generator=torch.Generator().manual_seed(5))
+    shuffled = W.ParticleChunk(*(getattr(parts, k)[perm] for k in ("x", "y", "z", "ux", "uy", "uz", "w", "species")))
+    Js = []
+    for p in (parts, shuffled):
+        pic = PP.gpu_for(wl, p, fields)
+        pic.step(1)
+        Js.append(pic.get_current().cpu().numpy().astype(np.float64))
+        pic.destroy()
+    assert np.abs(Js[0]).max() > 0 and np.array_equal(Js[0], Js[1])
+
+
 @pytest.mark.parametrize("name", ["cfg1_tiny_cic", "cfg2_thermal_tsc_32", "cfg4_khi_hotspot_tsc_24", "cfg5_pqs_32x32x16"])
 def test_ten_steps_free_running(name):
     rep, pic, wl = _run(name, 10)
