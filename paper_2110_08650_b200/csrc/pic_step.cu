@@ -199,7 +199,7 @@ __device__ __forceinline__ void deposit1(float* jt, int* jhi, int* jlo, int base
                 if (a == W - 2 && !lane_wa) acc = 0.0f;
                 const int off = base + a * sa + b * sb + c * sc;
                 if (FIX) {
-                    fix_add(jhi, jlo, off, acc);
+                    fix_add(jhi, jlo, off, acc);   // (predicating zero adds was measured slower: 6.0 vs 6.7e9)
                 } else {
                     if (acc != 0.0f) atomicAdd(jt + off, acc);
                 }
