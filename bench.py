@@ -118,6 +118,21 @@ def oracle_sample_rate(wl, n_sample: int, n_steps: int = 1):
     return orc.n * n_steps / dt, dt, orc.n
 
 
+def reduce_max_over_ranks(values, device, world: int):
+    """MAX over ranks of a list of floats (device time of the slowest rank decides); identity at N=1."""
+    import torch
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def whole_job_value(world: int, particles_per_rank: int, steps: int, seconds: float) -> float:
+    """Replicas only: every rank steps its own copy of the workload; units of all ranks / slowest time."""
+    return world * particles_per_rank * steps / seconds
+
+
 def run_reference(args):
     """--impl reference: the oracle, as it stands, on the host cores; each step = one oracle step
     over a bounded sample of the workload (rank 0 only)."""
@@ -207,11 +222,8 @@ def run_ours(args):
     launches = pic.launch_count() - l0
     pic.set_option("timing", 0)
     stats = pic.get_stats()
-    t = torch.tensor([ms, kernel_ms / max(n_kernel, 1)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max, kernel_ms_avg = float(t[0]), float(t[1])
-    value = world * n * K / (ms_max * 1e-3)
+    ms_max, kernel_ms_avg = reduce_max_over_ranks([ms, kernel_ms / max(n_kernel, 1)], dev, world)
+    value = whole_job_value(world, n, K, ms_max * 1e-3)
     pic.destroy()
 
     # ---------------------------------------------------------------- end to end with host buffers
@@ -253,10 +265,7 @@ def run_ours(args):
         e2e_step()
     barrier()
     e2e_s = time.perf_counter() - t0
-    te = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_value = world * n * e2e_steps / float(te[0])
+    e2e_value = whole_job_value(world, n, e2e_steps, reduce_max_over_ranks([e2e_s], dev, world)[0])
 
     if rank == 0:
         peak, peak_src = measured_peaks()

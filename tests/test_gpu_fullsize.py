@@ -1,0 +1,103 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times, on sampled outputs
+the oracle can compute one by one (particles are independent: E,B static, J does not feed back):
+  * a random sample of particles: positions, momenta, membership after one step;
+  * J inside a sub-box: the oracle deposits every particle that can reach it;
+  * properties that hold at any size: ids are a permutation, counts sum, membership == floor(X) div SC.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import pic_parity as PP
+from paper_2110_08650_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+BOX_LO, BOX_HI, MARGIN = 40, 56, 4     # J compared in [44,52)^3; sources taken from [40,56)^3
+
+
+def _fullsize(name, u_scale, per_chunk_sample=1500):
+    from paper_2110_08650_b200.binding import Pic
+    wl = W.CONFIGS[name]
+    n = W.n_particles(wl)
+    dev = "cuda:0"
+    fields = W.make_fields(wl, device=dev)
+    pic = Pic(wl.grid, wl.cell, wl.dt, wl.supercell, wl.shape_order, max_particles=n, device=dev)
+    keys = ("x", "y", "z", "ux", "uy", "uz", "w", "species")
+    samp = {k: [] for k in keys}
+    box = {k: [] for k in keys}
+    samp_ids, id0 = [], 0
+    g = torch.Generator(device=dev).manual_seed(11)
+    for chunk in W.particle_chunks(wl, device=dev, max_chunk=1 << 23):
+        pic.load_particles(*(getattr(chunk, k) for k in keys))
+        sel = torch.randperm(chunk.n, generator=g, device=dev)[:per_chunk_sample]
+        inb = torch.ones(chunk.n, dtype=torch.bool, device=dev)
+        for k in "xyz":
+            c = getattr(chunk, k)
+            inb &= (c >= BOX_LO) & (c < BOX_HI)
+        for k in keys:
+            samp[k].append(getattr(chunk, k)[sel].cpu())
+            box[k].append(getattr(chunk, k)[inb].cpu())
+        samp_ids.append((sel + id0).cpu())
+        id0 += chunk.n
+        pic.sync()
+    pic.set_fields(fields)
+    pic.step(1)
+    pic.sync()
+    st = pic.get_stats()
+    assert st["error"] == 0 and st["particles"] == n
+    # ---- properties at any size
+    P = pic.get_particles()
+    ids = P["id"].to(torch.int64) & 0xFFFFFFFF
+    order = torch.argsort(ids)
+    assert torch.equal(ids[order], torch.arange(n, device=dev))
+    assert int(pic.get_counts().sum()) == n
+    assert PP.gpu_membership_consistent(wl, pic)
+    # ---- sampled particles
+    samp = {k: torch.cat(v) for k, v in samp.items()}
+    sid = torch.cat(samp_ids).to(dev)
+    fh = fields.cpu()
+    orc = oracle.Oracle(wl.grid, wl.cell, wl.dt, wl.supercell, wl.shape_order)
+    orc.load_particles(*(samp[k].numpy() for k in keys[:7]), species=samp["species"].numpy())
+    orc.set_fields(fh.numpy())
+    assert orc.step(1) == 0
+    O = orc.particles()
+    rows = order[sid]
+    worst_x, worst_u, mism = 0.0, 0.0, 0
+    near = np.zeros(sid.numel(), dtype=bool)
+    for a, k in enumerate("xyz"):
+        d = P[k][rows].cpu().numpy() - O[k]
+        d -= wl.grid[a] * np.round(d / wl.grid[a])
+        worst_x = max(worst_x, float(np.abs(d).max()))
+        face = O[k] / wl.supercell[a]
+        near |= np.abs(face - np.round(face)) * wl.supercell[a] <= PP.BAND
+    du = np.sqrt(sum((P[k][rows].cpu().numpy().astype(np.float64) - O[k]) ** 2 for k in ("ux", "uy", "uz")))
+    un = np.sqrt(sum(O[k] ** 2 for k in ("ux", "uy", "uz")))
+    worst_u = float((du / np.maximum(un, u_scale)).max())
+    mism = int(((P["supercell"][rows].cpu().numpy() != O["supercell"]) & ~near).sum())
+    # ---- J in the sub-box
+    box = {k: torch.cat(v) for k, v in box.items()}
+    ob = oracle.Oracle(wl.grid, wl.cell, wl.dt, wl.supercell, wl.shape_order)
+    ob.load_particles(*(box[k].numpy() for k in keys[:7]), species=box["species"].numpy())
+    ob.set_fields(fh.numpy())
+    assert ob.step(1) == 0
+    lo, hi = BOX_LO + MARGIN, BOX_HI - MARGIN
+    Jg = pic.get_current()[:, lo:hi, lo:hi, lo:hi].cpu().numpy().astype(np.float64)
+    Jo = np.stack(ob.J)[:, lo:hi, lo:hi, lo:hi]
+    jmax = float(pic.get_current().abs().max())
+    j_err = float(np.abs(Jg - Jo).max() / jmax)
+    print(f"\n[{name} full size, n={n}] sample {sid.numel()}: max|dX|={worst_x:.3e} max|du|/scale={worst_u:.3e} "
+          f"membership mismatches={mism} (near-face {int(near.sum())}); J sub-box from {box['x'].numel()} particles: "
+          f"err/max|J|={j_err:.3e}; leavers={st['leavers_last']} max_count={st['max_count']}")
+    assert worst_x <= PP.TOL_X and worst_u <= PP.TOL_U and mism == 0 and j_err <= PP.TOL_J1
+    pic.destroy()
+
+
+def test_config2_thermal_128_full_size():
+    _fullsize("thermal_128", 0.05)
+
+
+def test_config4_khi_hotspot_full_size():
+    """63.7 M particles, 276 supercells with ~115 k particles each (450 frames per CTA)."""
+    _fullsize("khi_hotspot", 0.01, per_chunk_sample=800)
