@@ -163,6 +163,54 @@ def run_reference(args):
     }))
 
 
+def measure_e2e(args, wl, n, K, fields, fresh, barrier, dev, world):
+    """The same metric through the C ABI with HOST buffers: every step copies the inputs from pinned
+    host memory, loads, steps once and reads J and the particles back to the host."""
+    import torch
+    from paper_2110_08650_b200 import workloads as W
+    e2e_steps = min(K, args.e2e_steps)
+    names = ("x", "y", "z", "ux", "uy", "uz", "w", "species")
+    host = {k: [] for k in names}
+    for chunk in W.particle_chunks(wl, device=dev, max_chunk=1 << 23):
+        for k in names:
+            host[k].append(getattr(chunk, k).cpu())
+    host = {k: torch.cat(v).pin_memory() for k, v in host.items()}
+    host_fields = fields.cpu().pin_memory()
+    dev_in = {k: torch.empty_like(v, device=dev) for k, v in host.items()}
+    dev_fields = torch.empty_like(fields)
+    out_keys = ("x", "y", "z", "ux", "uy", "uz")
+    host_out = {k: torch.empty(n, dtype=host[k].dtype).pin_memory() for k in out_keys}
+    host_J = torch.empty((3,) + tuple(fields.shape[1:]), dtype=torch.float32).pin_memory()
+    h2d = sum(v.numel() * v.element_size() for v in host.values()) + host_fields.numel() * 4
+    d2h = sum(v.numel() * v.element_size() for v in host_out.values()) + host_J.numel() * 4
+
+    def e2e_step():
+        p = fresh()
+        for k in names:
+            dev_in[k].copy_(host[k], non_blocking=True)
+        dev_fields.copy_(host_fields, non_blocking=True)
+        p.load_particles(*(dev_in[k] for k in names))
+        p.set_fields(dev_fields)
+        p.step(1)
+        host_J.copy_(p.get_current(), non_blocking=True)
+        P = p.get_particles(n)
+        for k in out_keys:
+            host_out[k].copy_(P[k], non_blocking=True)
+        torch.cuda.synchronize()
+        p.destroy()
+
+    e2e_step()                      # warm-up (page-locking, allocator)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_step()
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    e2e_value = whole_job_value(world, n, e2e_steps, reduce_max_over_ranks([e2e_s], dev, world)[0])
+
+    return {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -226,46 +274,7 @@ def run_ours(args):
     value = whole_job_value(world, n, K, ms_max * 1e-3)
     pic.destroy()
 
-    # ---------------------------------------------------------------- end to end with host buffers
-    e2e_steps = min(K, args.e2e_steps)
-    names = ("x", "y", "z", "ux", "uy", "uz", "w", "species")
-    host = {k: [] for k in names}
-    for chunk in W.particle_chunks(wl, device=dev, max_chunk=1 << 23):
-        for k in names:
-            host[k].append(getattr(chunk, k).cpu())
-    host = {k: torch.cat(v).pin_memory() for k, v in host.items()}
-    host_fields = fields.cpu().pin_memory()
-    dev_in = {k: torch.empty_like(v, device=dev) for k, v in host.items()}
-    dev_fields = torch.empty_like(fields)
-    out_keys = ("x", "y", "z", "ux", "uy", "uz")
-    host_out = {k: torch.empty(n, dtype=host[k].dtype).pin_memory() for k in out_keys}
-    host_J = torch.empty((3,) + tuple(fields.shape[1:]), dtype=torch.float32).pin_memory()
-    h2d = sum(v.numel() * v.element_size() for v in host.values()) + host_fields.numel() * 4
-    d2h = sum(v.numel() * v.element_size() for v in host_out.values()) + host_J.numel() * 4
-
-    def e2e_step():
-        p = fresh()
-        for k in names:
-            dev_in[k].copy_(host[k], non_blocking=True)
-        dev_fields.copy_(host_fields, non_blocking=True)
-        p.load_particles(*(dev_in[k] for k in names))
-        p.set_fields(dev_fields)
-        p.step(1)
-        host_J.copy_(p.get_current(), non_blocking=True)
-        P = p.get_particles(n)
-        for k in out_keys:
-            host_out[k].copy_(P[k], non_blocking=True)
-        torch.cuda.synchronize()
-        p.destroy()
-
-    e2e_step()                      # warm-up (page-locking, allocator)
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        e2e_step()
-    barrier()
-    e2e_s = time.perf_counter() - t0
-    e2e_value = whole_job_value(world, n, e2e_steps, reduce_max_over_ranks([e2e_s], dev, world)[0])
+    e2e = measure_e2e(args, wl, n, K, fields, fresh, barrier, dev, world) if args.e2e_steps > 0 else None
 
     if rank == 0:
         peak, peak_src = measured_peaks()
@@ -301,8 +310,7 @@ def run_ours(args):
                          "frac_of_8000_GBps": achieved / 8000.0,
                          "kernel_share_of_step": kernel_ms_avg / (ms_max / K)},
             "cpu_baseline": cpu,
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "steps": e2e_steps},
+            "e2e": e2e,
             "gpu_launches": launches, "clocks": clocks,
         }))
     if world > 1:
