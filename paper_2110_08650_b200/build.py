@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpic_b200.so")
 SOURCES = ("pic_api.cu", "pic_step.cu")
-HEADERS = ("pic_internal.cuh", os.path.join("..", "..", "include", "pic_b200.h"))
+HEADERS = ("pic_internal.cuh", "pic_device.cuh", os.path.join("..", "..", "include", "pic_b200.h"))
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "--use_fast_math=false",

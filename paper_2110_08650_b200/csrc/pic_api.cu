@@ -41,8 +41,8 @@ static std::string g_create_error;
 namespace {
 
 struct Layout {
-    uint64_t pos, mom, pid, tbl_pool, tbl_off, tbl_cap, sc_nframes, sc_count, sc_stay, sc_incoming,
-        x_pos, x_mom, x_id, x_dst, ctr, ctr64, F, Fpad, J, J64, sc_offset, total;
+    uint64_t rec0, rec1, pid0, pid1, tbl_pool, tbl_off, tbl_cap, sc_nframes, sc_count, sc_tail, sc_incoming,
+        cell_off, cell_hist, cell_perm, cell_kbase, x_rec, x_id, x_dst, ctr, ctr64, F, Fpad, J, J64, sc_offset, total;
     int n_frames, tbl_pool_size, x_cap, nsc;
 };
 
@@ -67,18 +67,22 @@ int compute_layout(const int32_t grid[3], const int32_t sc[3], int order, int64_
     if (n_frames > 0x7fffffffull / 2 || tblp > 0x7fffffffull || xcap > 0x7fffffffull) return PIC_EINVAL;
     uint64_t o = 0;
     auto take = [&](uint64_t bytes) { uint64_t r = o; o = align_up(o + bytes, 256); return r; };
-    L->pos = take(slots * 16);
-    L->mom = take(slots * 16);
-    L->pid = take(slots * 4);
+    L->rec0 = take(slots * 32);
+    L->rec1 = take(slots * 32);
+    L->pid0 = take(slots * 4);
+    L->pid1 = take(slots * 4);
     L->tbl_pool = take(tblp * 4);
     L->tbl_off = take(nsc * 4);
     L->tbl_cap = take(nsc * 4);
     L->sc_nframes = take(nsc * 4);
     L->sc_count = take(nsc * 4);
-    L->sc_stay = take(nsc * 4);
+    L->sc_tail = take(nsc * 4);
     L->sc_incoming = take(nsc * 4);
-    L->x_pos = take(xcap * 16);
-    L->x_mom = take(xcap * 16);
+    L->cell_off = take(nsc * 257 * 4);
+    L->cell_hist = take(nsc * 256 * 4);
+    L->cell_perm = take(nsc * 256);
+    L->cell_kbase = take(nsc * 256 * 2);
+    L->x_rec = take(xcap * 32);
     L->x_id = take(xcap * 4);
     L->x_dst = take(xcap * 4);
     L->ctr = take(CTR_N * 4);
@@ -153,6 +157,7 @@ __global__ void pic_load_count_kernel(const PicDev d, const LoadArgs a)
         int lc;
         int s = load_locate(d, a, i, P, lc);
         atomicAdd(d.sc_incoming + s, 1);
+        atomicAdd(d.cell_hist + (size_t)s * 256 + lc, 1);
         atomicMax(d.ctr + CTR_WMAX_BITS, __float_as_int(fabsf(a.w[i])));
     }
 }
@@ -165,22 +170,25 @@ __global__ void pic_load_scatter_kernel(const PicDev d, const LoadArgs a)
         int lc;
         const int s = load_locate(d, a, i, P, lc);
         const int sp = a.species ? a.species[i] : 0;
-        const int slot = atomicAdd(d.sc_count + s, 1);
+        const int slot = atomicAdd(d.sc_tail + s, 1);
         const int fr = slot >> 8;
         if (fr < d.sc_nframes[s]) {
             const size_t idx = (size_t)d.tbl_pool[d.tbl_off[s] + fr] * PIC_FRAME + (slot & (PIC_FRAME - 1));
-            d.pos[idx] = P;
-            d.mom[idx] = make_float4(a.ux[i], a.uy[i], a.uz[i],
-                                     __uint_as_float(pic_pack_bits(lc, sp & (PIC_NSPECIES - 1))));
-            d.pid[idx] = a.id0 + (unsigned)i;
+            d.rec[d.cur][2 * idx] = P;
+            d.rec[d.cur][2 * idx + 1] = make_float4(a.ux[i], a.uy[i], a.uz[i],
+                                                    __uint_as_float(pic_pack_bits(lc, sp & (PIC_NSPECIES - 1))));
+            d.pid[d.cur][idx] = a.id0 + (unsigned)i;
         }
     }
 }
 
-__global__ void pic_copy_int_kernel(int* dst, const int* src, int n)
+// Before an appending load is sorted in: count the particles already present per cell.
+__global__ void pic_hist_add_present_kernel(const PicDev d)
 {
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) dst[i] = src[i];
+    const size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
+    if (i >= (size_t)d.nsc * 256) return;
+    const size_t s = i >> 8, c = i & 255;
+    d.cell_hist[i] += d.cell_off[s * 257 + c + 1] - d.cell_off[s * 257 + c];
 }
 
 // ------------------------------------------------------------------ read-back kernels
@@ -225,8 +233,8 @@ __global__ void pic_get_particles_kernel(const PicDev d, const GetArgs a)
         const long long o = off + slot;
         if (o >= a.capacity) break;
         const size_t idx = (size_t)tbl[slot >> 8] * PIC_FRAME + (slot & (PIC_FRAME - 1));
-        const float4 P = d.pos[idx];
-        const float4 M = d.mom[idx];
+        const float4 P = d.rec[d.cur][2 * idx];
+        const float4 M = d.rec[d.cur][2 * idx + 1];
         const uint32_t bits = __float_as_uint(M.w);
         const int lc = bits & 0xffff;
         if (a.x) a.x[o] = ((double)(ox + (lc & 7)) + (double)P.x) * a.cx;
@@ -237,7 +245,7 @@ __global__ void pic_get_particles_kernel(const PicDev d, const GetArgs a)
         if (a.uz) a.uz[o] = M.z;
         if (a.w) a.w[o] = P.w;
         if (a.species) a.species[o] = (bits >> 16) & 0xff;
-        if (a.id) a.id[o] = d.pid[idx];
+        if (a.id) a.id[o] = d.pid[d.cur][idx];
         if (a.supercell) a.supercell[o] = s;
     }
 }
@@ -379,21 +387,26 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     d.jfx = (float)(cell[0] / dt / V); d.jfy = (float)(cell[1] / dt / V); d.jfz = (float)(cell[2] / dt / V);
     refresh_species(c);
     char* w = c->ws;
-    d.pos = (float4*)(w + L.pos); d.mom = (float4*)(w + L.mom); d.pid = (uint32_t*)(w + L.pid);
+    d.rec[0] = (float4*)(w + L.rec0); d.rec[1] = (float4*)(w + L.rec1);
+    d.pid[0] = (uint32_t*)(w + L.pid0); d.pid[1] = (uint32_t*)(w + L.pid1);
+    d.cur = 0;
     d.n_frames = L.n_frames;
     d.tbl_pool = (int*)(w + L.tbl_pool); d.tbl_pool_size = L.tbl_pool_size;
     d.tbl_off = (int*)(w + L.tbl_off); d.tbl_cap = (int*)(w + L.tbl_cap);
     d.sc_nframes = (int*)(w + L.sc_nframes); d.sc_count = (int*)(w + L.sc_count);
-    d.sc_stay = (int*)(w + L.sc_stay); d.sc_incoming = (int*)(w + L.sc_incoming);
-    d.x_pos = (float4*)(w + L.x_pos); d.x_mom = (float4*)(w + L.x_mom);
+    d.sc_tail = (int*)(w + L.sc_tail); d.sc_incoming = (int*)(w + L.sc_incoming);
+    d.cell_off = (int*)(w + L.cell_off); d.cell_hist = (int*)(w + L.cell_hist);
+    d.cell_perm = (unsigned char*)(w + L.cell_perm);
+    d.cell_kbase = (unsigned short*)(w + L.cell_kbase);
+    d.x_rec = (float4*)(w + L.x_rec);
     d.x_id = (uint32_t*)(w + L.x_id); d.x_dst = (int*)(w + L.x_dst); d.x_cap = L.x_cap;
     d.ctr = (int*)(w + L.ctr); d.ctr64 = (unsigned long long*)(w + L.ctr64);
     d.F = (const float*)(w + L.F); d.Fpad = (const float*)(w + L.Fpad); d.J = (float*)(w + L.J); d.J64 = (long long*)(w + L.J64);
     d.sc_offset = (long long*)(w + L.sc_offset);
     d.pad_lo_x = (shape_order == 3) ? 2 : 1;
 
-    // zero the bookkeeping region [tbl_off, x_pos) and the counters, J
-    cudaError_t e = cudaMemsetAsync(w + L.tbl_off, 0, L.x_pos - L.tbl_off, c->stream);
+    // zero the bookkeeping region [tbl_off, x_rec) and the counters, J
+    cudaError_t e = cudaMemsetAsync(w + L.tbl_off, 0, L.x_rec - L.tbl_off, c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(w + L.ctr, 0, L.F - L.ctr, c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(w + L.J, 0, L.sc_offset - L.J, c->stream);
     if (e != cudaSuccess) { int r = cuda_fail(nullptr, e, "pic_create: cudaMemsetAsync"); delete c; return r; }
@@ -429,15 +442,18 @@ int32_t pic_load_particles(pic_ctx* c, int64_t n, const double* x, const double*
     a.icx = 1.0 / c->cell[0]; a.icy = 1.0 / c->cell[1]; a.icz = 1.0 / c->cell[2];
     const PicDev& d = c->d;
     const int grid = (int)((n + 255) / 256 < 148 * 16 ? (n + 255) / 256 : 148 * 16);
+    // count per supercell and per cell (new + already present), make room, append, sort in
     pic_load_count_kernel<<<grid, 256, 0, c->stream>>>(d, a);
-    pic_copy_int_kernel<<<(d.nsc + 255) / 256, 256, 0, c->stream>>>(d.sc_stay, d.sc_count, d.nsc);
+    pic_hist_add_present_kernel<<<(unsigned)(((size_t)d.nsc * 256 + 255) / 256), 256, 0, c->stream>>>(d);
     c->launches += 2;
-    cudaError_t e = pic_launch_resort(d, c->stream, &c->launches, false);   // frame allocation only
+    cudaError_t e = pic_launch_prepare(d, c->stream, &c->launches);
     if (e != cudaSuccess) return cuda_fail(c, e, "pic_load_particles: prepare");
     pic_load_scatter_kernel<<<grid, 256, 0, c->stream>>>(d, a);
     c->launches += 1;
     e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(c, e, "pic_load_particles: scatter");
+    if (e == cudaSuccess) e = pic_launch_sort(d, c->stream, &c->launches);
+    if (e != cudaSuccess) return cuda_fail(c, e, "pic_load_particles: scatter/sort");
+    c->d.cur ^= 1;
     c->n_particles += n;
     return PIC_OK;
 }
@@ -465,7 +481,7 @@ int32_t pic_set_fields(pic_ctx* c, const float* Ex, const float* Ey, const float
 
 static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
 {
-    const PicDev& d = c->d;
+    PicDev& d = c->d;
     const size_t ncell = (size_t)d.nx * d.ny * d.nz;
     for (int i = 0; i < n; ++i) {
         cudaError_t e = c->fixed_point ? cudaMemsetAsync(d.J64, 0, 3 * ncell * sizeof(long long), st)   // S16
@@ -483,8 +499,12 @@ static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
             c->events.push_back(ev0);
             c->events.push_back(ev1);
         }
-        if (e == cudaSuccess) e = pic_launch_resort(d, st, &c->launches, true);
+        if (e == cudaSuccess && c->fixed_point) e = pic_launch_convert(d, st, &c->launches);
+        if (e == cudaSuccess) e = pic_launch_prepare(d, st, &c->launches);
+        if (e == cudaSuccess) e = pic_launch_scatter(d, st, &c->launches);
+        if (e == cudaSuccess) e = pic_launch_sort(d, st, &c->launches);
         if (e != cudaSuccess) return cuda_fail(c, e, "pic_step: launch");
+        d.cur ^= 1;     // the sorted state now lives in the other pool
     }
     return PIC_OK;
 }

@@ -3,11 +3,14 @@
 //
 // Particle storage ("per-supercell ... fixed-sized
 // particle vectors"): a pool of FRAMES of PIC_FRAME slots.  A frame belongs to one
-// supercell; a supercell's particles occupy slots [0,count) of its frame list, densely.
-// Per slot: float4 pos = {fx,fy,fz,w} (in-cell fraction in [0,1), weight),
-//           float4 mom = {ux,uy,uz, bits(local cell | species<<16)},
-//           uint32  id.
-// The frame list of supercell s is tbl_pool[tbl_off[s] .. tbl_off[s]+sc_nframes[s]).
+// supercell; a supercell's particles occupy slots [0,count) of its frame list, SORTED BY
+// CELL (cell_off[s][c] .. cell_off[s][c+1] are the slots of local cell c).  Per slot one
+// 32-byte record (one DRAM sector): float4 {fx,fy,fz,w} (in-cell fraction in [0,1), weight)
+// and float4 {ux,uy,uz, bits(local cell | species<<16 | flags<<24)}, plus a uint32 id in a
+// parallel array.  Two pools (ping-pong): the step kernel updates records in place in pool
+// `cur`, the sort kernel writes the re-sorted supercell into the other pool.
+// The frame list of supercell s is tbl_pool[tbl_off[s] .. tbl_off[s]+sc_nframes[s]), the same
+// frame indices in both pools.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -18,6 +21,7 @@
 #define PIC_SCZ 4
 #define PIC_SC_CELLS (PIC_SCX * PIC_SCY * PIC_SCZ)
 #define PIC_NSPECIES 16
+#define PIC_LEFT_FLAG 0x01000000u   // record bits: the particle left this supercell (hole until the sort)
 
 // device counters (int32 each) in PicDev::ctr
 enum {
@@ -42,10 +46,10 @@ struct PicDev {
     float h[PIC_NSPECIES];       // (q/m) dt / 2
     float q[PIC_NSPECIES];
     float qmax;                  // max |q| over the species table
-    // frames
-    float4* pos;
-    float4* mom;
-    uint32_t* pid;
+    // frames (two pools, see above)
+    float4* rec[2];
+    uint32_t* pid[2];
+    int cur;                     // pool holding the current state
     int n_frames;
     int* tbl_pool;
     int tbl_pool_size;
@@ -53,11 +57,14 @@ struct PicDev {
     int* tbl_cap;                // [nsc]
     int* sc_nframes;             // [nsc]
     int* sc_count;               // [nsc] particles in the supercell
-    int* sc_stay;                // [nsc] stayers after the step kernel's compaction
+    int* sc_tail;                // [nsc] slots in use incl. holes of leavers and appended arrivals
+    int* cell_off;               // [nsc][257] slot ranges of the local cells (sorted arrangement)
+    int* cell_hist;              // [nsc][256] particles per NEW local cell (stayers + arrivals), zero between steps
+    unsigned char* cell_perm;    // [nsc][256] local cells ordered by decreasing work-item length
+    unsigned short* cell_kbase;  // [nsc][256] first work item of the cell at that position
     int* sc_incoming;            // [nsc] leavers headed here
     // exchange buffer for supercell leavers
-    float4* x_pos;
-    float4* x_mom;
+    float4* x_rec;               // 2 float4 per entry
     uint32_t* x_id;
     int* x_dst;
     int x_cap;
@@ -81,6 +88,14 @@ struct PicDev {
 #define PIC_PAD_Y 4
 #define PIC_PAD_Z 4
 
+// Work items of the step kernel: a cell of n particles is cut into ceil(n/T) segments, with T about
+// 3/4 of the supercell's mean cell population (measured optimum of balance vs. flushes).
+__host__ __device__ inline int pic_segment_target(int supercell_count)
+{
+    const int t = (3 * supercell_count + 1023) / 1024;
+    return t < 4 ? 4 : t;
+}
+
 __host__ __device__ inline uint32_t pic_pack_bits(int local_cell, int species)
 {
     return (uint32_t)local_cell | ((uint32_t)species << 16);
@@ -89,4 +104,7 @@ __host__ __device__ inline uint32_t pic_pack_bits(int local_cell, int species)
 // launchers implemented in pic_step.cu
 cudaError_t pic_launch_step(const PicDev& d, int order, bool use_tma, bool fixed_point, const void* tmap,
                             cudaStream_t st, int64_t* launches);
-cudaError_t pic_launch_resort(const PicDev& d, cudaStream_t st, int64_t* launches, bool scatter);
+cudaError_t pic_launch_convert(const PicDev& d, cudaStream_t st, int64_t* launches);
+cudaError_t pic_launch_prepare(const PicDev& d, cudaStream_t st, int64_t* launches);
+cudaError_t pic_launch_scatter(const PicDev& d, cudaStream_t st, int64_t* launches);
+cudaError_t pic_launch_sort(const PicDev& d, cudaStream_t st, int64_t* launches);   // pool cur -> the other

@@ -28,10 +28,10 @@ def test_library_loads_and_exports_every_symbol():
 
 
 def test_workspace_bytes_validation_and_size():
-    # config 2: 33.5M particles -> two float4 + one u32 per slot, ~1.25 GB of frames
+    # config 2: 33.5M particles -> 32 B record + u32 id per slot, two pools, ~2.7 GB
     n = 128 ** 3 * 16
     b = binding.workspace_bytes((128, 128, 128), (8, 8, 4), 2, n)
-    assert 36 * n < b < 2.2 * 36 * n
+    assert 2 * 36 * n < b < 3.2 * 36 * n      # two pools of 36 B slots + grids + bookkeeping
     with pytest.raises(binding.PicError) as e:
         binding.workspace_bytes((100, 128, 128), (8, 8, 4), 2, n)
     assert e.value.code == binding.PIC_EINVAL

@@ -61,10 +61,9 @@ def test_float_atomic_deposit_variant(name):
     pic.destroy()
 
 
-def test_fixed_point_tile_is_order_independent():
-    """Fixed-point accumulation (shared tile and global J) is exact integer arithmetic: two runs whose
-    particles are loaded in different orders (different thread assignment and atomic order) give
-    bit-identical J."""
+def test_load_order_changes_J_only_by_rounding():
+    """Two runs whose particles are loaded in different orders differ only by the fp32 rounding of the
+    per-cell register sums (the shared tile and global J accumulate exactly, in fixed point)."""
     wl, _ = CASES["cfg2_thermal_tsc_32"]
     parts, fields = W.make_particles(wl), W.make_fields(wl)
     perm = torch.randperm(parts.n, generator=torch.Generator().manual_seed(5))
@@ -75,7 +74,8 @@ def test_fixed_point_tile_is_order_independent():
         pic.step(1)
         Js.append(pic.get_current().cpu().numpy().astype(np.float64))
         pic.destroy()
-    assert np.abs(Js[0]).max() > 0 and np.array_equal(Js[0], Js[1])
+    scale = np.abs(Js[0]).max()
+    assert scale > 0 and np.abs(Js[0] - Js[1]).max() <= 1e-6 * scale
 
 
 @pytest.mark.parametrize("name", ["cfg1_tiny_cic", "cfg2_thermal_tsc_32", "cfg4_khi_hotspot_tsc_24", "cfg5_pqs_32x32x16"])
