@@ -241,6 +241,7 @@ def run_ours(args):
         pic = Pic(wl.grid, wl.cell, wl.dt, wl.supercell, wl.shape_order, max_particles=n, device=dev, workspace=ws)
         pic.set_option("tma", args.tma)
         pic.set_option("deposit", args.deposit)
+        pic.set_option("segment", args.segment)
         return pic
 
     # ---------------------------------------------------------------- device-resident throughput
@@ -326,6 +327,7 @@ def main():
     ap.add_argument("--workload", default="thermal_128")
     ap.add_argument("--tma", type=int, default=1)
     ap.add_argument("--deposit", type=int, default=1, help="1 fixed-point integer atomics, 0 float CAS atomics")
+    ap.add_argument("--segment", type=int, default=3, help="work-item length in quarters of the mean cell population")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -50,6 +50,7 @@ struct PicDev {
     float4* rec[2];
     uint32_t* pid[2];
     int cur;                     // pool holding the current state
+    int seg_num;                 // work-item length target in quarters of the mean cell population (2..16)
     int n_frames;
     int* tbl_pool;
     int tbl_pool_size;
@@ -90,9 +91,9 @@ struct PicDev {
 
 // Work items of the step kernel: a cell of n particles is cut into ceil(n/T) segments, with T about
 // 3/4 of the supercell's mean cell population (measured optimum of balance vs. flushes).
-__host__ __device__ inline int pic_segment_target(int supercell_count)
+__host__ __device__ inline int pic_segment_target(int supercell_count, int seg_num)
 {
-    const int t = (3 * supercell_count + 1023) / 1024;
+    const int t = (seg_num * supercell_count + 1023) / 1024;     // seg_num/4 of the mean cell population
     return t < 4 ? 4 : t;
 }
 

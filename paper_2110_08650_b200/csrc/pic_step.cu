@@ -19,7 +19,8 @@ namespace {
 #define PIC_XSTAGE 256     // leavers staged in shared memory per CTA before one bulk append
 #define PIC_SLOWCAP 768    // queued out-of-window particles per CTA
 #define PIC_STEP_THREADS 128   // 2 CTAs of 4 warps per SM: ~250 registers per thread for the accumulators
-#define PIC_ITEMCAP 640    // work items (cell segments) per supercell: <= 256 + count/T, T >= 0.75 * count/256
+#define PIC_DIRECT_BELOW 1536   // supercells with fewer particles (< 6 per cell) take the per-particle path
+#define PIC_ITEMCAP 800    // work items (cell segments) per supercell: <= 256 + count/T, T >= count/512
 
 // Esirkepov density decomposition of one component, straight into the
 // shared tile, with a per-particle window [lo, lo+O+2):
@@ -148,10 +149,131 @@ __device__ __forceinline__ void flush1(float* sJ, int* sJhi, int* sJlo, int off,
     else if (v != 0.0f) atomicAdd(sJ + off, v);
 }
 
-// ------------------------------------------------------------------ the step kernel
-template <int O, bool TMA, bool FIX>
-__global__ void __launch_bounds__(PIC_STEP_THREADS, 2) pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
+// a2 + a3 for one particle: gather E,B at x^n, Boris push (step 4), move
+// (step 5) and the split of the new position into cell shift + in-cell fraction (reading S19).
+template <int O>
+__device__ __forceinline__ void push_particle(const PicDev& d, const float* sF, int cx, int cy, int cz, int sp,
+                                              const float4& P, const float4& M, float (&un)[3], float (&fn)[3],
+                                              float (&x1)[3], int (&sh)[3])
 {
+    using G = Geo<O>;
+    // ---- a2: gather at x^n
+    float E[3], B[3];
+    {
+        float wu[3][O + 1], ws[3][O + 1];
+        int bu[3], bs[3];
+        const float f[3] = {P.x, P.y, P.z};
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            bu[a] = shape<O>(f[a], wu[a]);
+            bs[a] = shape<O>(f[a] - 0.5f, ws[a]);
+        }
+        const int ux_ = cx + bu[0] + G::FL, sx_ = cx + bs[0] + G::FL;
+        const int uy_ = (cy + bu[1] + G::FL) * G::FPX, sy_ = (cy + bs[1] + G::FL) * G::FPX;
+        const int uz_ = (cz + bu[2] + G::FL) * G::FPX * G::FNY, sz_ = (cz + bs[2] + G::FL) * G::FPX * G::FNY;
+        E[0] = gather1<O>(sF + 0 * G::FCOMP + sx_ + uy_ + uz_, ws[0], wu[1], wu[2]);
+        E[1] = gather1<O>(sF + 1 * G::FCOMP + ux_ + sy_ + uz_, wu[0], ws[1], wu[2]);
+        E[2] = gather1<O>(sF + 2 * G::FCOMP + ux_ + uy_ + sz_, wu[0], wu[1], ws[2]);
+        B[0] = gather1<O>(sF + 3 * G::FCOMP + ux_ + sy_ + sz_, wu[0], ws[1], ws[2]);
+        B[1] = gather1<O>(sF + 4 * G::FCOMP + sx_ + uy_ + sz_, ws[0], wu[1], ws[2]);
+        B[2] = gather1<O>(sF + 5 * G::FCOMP + sx_ + sy_ + uz_, ws[0], ws[1], wu[2]);
+    }
+
+    // ---- a3: Boris push and move (step 5)
+    const float h = d.h[sp];
+    const float umx = fmaf(h, E[0], M.x), umy = fmaf(h, E[1], M.y), umz = fmaf(h, E[2], M.z);
+    const float igm = rsqrtf(1.0f + umx * umx + umy * umy + umz * umz);
+    const float tx = h * B[0] * igm, ty = h * B[1] * igm, tz = h * B[2] * igm;
+    const float sfac = 2.0f / (1.0f + tx * tx + ty * ty + tz * tz);
+    const float upx = umx + (umy * tz - umz * ty);
+    const float upy = umy + (umz * tx - umx * tz);
+    const float upz = umz + (umx * ty - umy * tx);
+    const float sx2 = tx * sfac, sy2 = ty * sfac, sz2 = tz * sfac;
+    const float unx = fmaf(h, E[0], umx + (upy * sz2 - upz * sy2));
+    const float uny = fmaf(h, E[1], umy + (upz * sx2 - upx * sz2));
+    const float unz = fmaf(h, E[2], umz + (upx * sy2 - upy * sx2));
+    const float ig = rsqrtf(1.0f + unx * unx + uny * uny + unz * unz);
+    const float del[3] = {unx * ig * d.dtdx, uny * ig * d.dtdy, unz * ig * d.dtdz};
+
+    // new in-cell fraction and cell shift (reading S19)
+    const float f0[3] = {P.x, P.y, P.z};
+    bool far = false;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        float fp = f0[a] + del[a];
+        float fl = floorf(fp);
+        float g = fp - fl;
+        int shift = (int)fl;
+        if (g >= 1.0f) {            // tiny negative fp: fp + 1 rounded up to 1
+            g = 0.0f;
+            shift += 1;
+        }
+        far |= (shift < -1) | (shift > 1);
+        fn[a] = g;
+        sh[a] = shift;
+        x1[a] = (float)shift + g;   // new position relative to the OLD cell's origin node
+    }
+    if (far) atomicOr(d.ctr + CTR_ERROR, PIC_DEV_MOVED_TOO_FAR);
+    un[0] = unx; un[1] = uny; un[2] = unz;
+}
+
+// a5 for one particle: new local cell and destination supercell; stayers are written back in place
+// and counted per new cell, leavers leave a flagged hole and are staged for the exchange buffer.
+__device__ __forceinline__ void finish_particle(const PicDev& d, float4* rec, size_t idx, int s, int ssx, int ssy, int ssz,
+                                                int cx, int cy, int cz, int sp, float4 P, float4 M,
+                                                const float (&un)[3], const float (&fn)[3], const int (&sh)[3],
+                                                int* s_hist, int* s_xn, float4* s_xrec, uint32_t* s_xid, int* s_xdst)
+{
+    const float unx = un[0], uny = un[1], unz = un[2];
+    // ---- a5: new cell, destination supercell, write back in place
+    int ncx = cx + sh[0], ncy = cy + sh[1], ncz = cz + sh[2];
+    const int dsx = (ncx < 0) ? -1 : (ncx >= PIC_SCX) ? 1 : 0;
+    const int dsy = (ncy < 0) ? -1 : (ncy >= PIC_SCY) ? 1 : 0;
+    const int dsz = (ncz < 0) ? -1 : (ncz >= PIC_SCZ) ? 1 : 0;
+    ncx -= dsx * PIC_SCX; ncy -= dsy * PIC_SCY; ncz -= dsz * PIC_SCZ;
+    const int nlc = ncx + PIC_SCX * (ncy + PIC_SCY * ncz);
+    const uint32_t nbits = pic_pack_bits(nlc, sp);
+    P.x = fn[0]; P.y = fn[1]; P.z = fn[2];
+    M.x = unx; M.y = uny; M.z = unz;
+    if ((dsx | dsy | dsz) == 0) {
+        M.w = __uint_as_float(nbits);
+        rec[2 * idx] = P;
+        rec[2 * idx + 1] = M;
+        atomicAdd(&s_hist[nlc], 1);
+    } else {
+        const int dst = wrapi(ssx + dsx, d.nsx) + d.nsx * (wrapi(ssy + dsy, d.nsy) + d.nsy * wrapi(ssz + dsz, d.nsz));
+        rec[2 * idx + 1] = make_float4(unx, uny, unz, __uint_as_float(nbits | PIC_LEFT_FLAG));   // hole
+        M.w = __uint_as_float(nbits);
+        const uint32_t id = d.pid[d.cur][idx];
+        const int k = atomicAdd(s_xn, 1);
+        if (k < PIC_XSTAGE) {
+            s_xrec[2 * k] = P; s_xrec[2 * k + 1] = M; s_xid[k] = id; s_xdst[k] = dst;
+        } else {                      // staging full: append directly
+            const int xs = atomicAdd(d.ctr + CTR_EXCH, 1);
+            if (xs < d.x_cap) {
+                d.x_rec[2 * (size_t)xs] = P; d.x_rec[2 * (size_t)xs + 1] = M; d.x_id[xs] = id; d.x_dst[xs] = dst;
+            } else {
+                atomicOr(d.ctr + CTR_ERROR, PIC_DEV_EXCHANGE_OVERFLOW);
+            }
+        }
+        atomicAdd(d.cell_hist + (size_t)dst * 256 + nlc, 1);
+        atomicAdd(d.sc_incoming + dst, 1);
+    }
+}
+
+// ------------------------------------------------------------------ the step kernel
+// SPARSE = false: supercells with >= PIC_DIRECT_BELOW particles, 128 threads, register sums per cell segment.
+// SPARSE = true : the others, 256 threads, one thread per particle straight into the tile.
+// Both variants are launched over all supercells; a CTA whose supercell belongs to the other one exits.
+template <int O, bool TMA, bool FIX, bool SPARSE>
+__global__ void __launch_bounds__(SPARSE ? 256 : PIC_STEP_THREADS, SPARSE ? 3 : 2)
+pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
+{
+    constexpr int NT = SPARSE ? 256 : PIC_STEP_THREADS;
+    {
+        const int n = d.sc_count[blockIdx.x];
+        if (n == 0 || (n < PIC_DIRECT_BELOW) != SPARSE) return;
+    }
     using G = Geo<O>;
     using S = StepSmem<O, FIX>;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -187,7 +309,7 @@ __global__ void __launch_bounds__(PIC_STEP_THREADS, 2) pic_step_kernel(const Pic
         }
     } else {
         const size_t ncell = (size_t)d.nx * d.ny * d.nz;
-        for (int e = tid; e < 6 * G::FNZ * G::FNY * G::FNX; e += PIC_STEP_THREADS) {
+        for (int e = tid; e < 6 * G::FNZ * G::FNY * G::FNX; e += NT) {
             int i = e % G::FNX;
             int r = e / G::FNX;
             int j = r % G::FNY;
@@ -200,9 +322,9 @@ __global__ void __launch_bounds__(PIC_STEP_THREADS, 2) pic_step_kernel(const Pic
                 __ldg(d.F + c * ncell + (size_t)gi + (size_t)d.nx * ((size_t)gj + (size_t)d.ny * gk));
         }
     }
-    for (int e = tid; e < NJ; e += PIC_STEP_THREADS) sJhi[e] = 0;
-    for (int t = tid; t < 257; t += PIC_STEP_THREADS) s_off[t] = d.cell_off[(size_t)s * 257 + t];
-    for (int t = tid; t < 256; t += PIC_STEP_THREADS) s_hist[t] = 0;
+    for (int e = tid; e < NJ; e += NT) sJhi[e] = 0;
+    for (int t = tid; t < 257; t += NT) s_off[t] = d.cell_off[(size_t)s * 257 + t];
+    for (int t = tid; t < 256; t += NT) s_hist[t] = 0;
     if (tid == 0) {
         s_xn = 0;
         s_slown = 0;
@@ -212,8 +334,9 @@ __global__ void __launch_bounds__(PIC_STEP_THREADS, 2) pic_step_kernel(const Pic
     // work items: every cell is cut into k = ceil(n/T) near-equal segments, T ~ 3/4 of the mean cell
     // population; cells come in the order the sort kernel fixed (by decreasing segment length), so
     // the 32 items a warp takes at a time hold similar numbers of particles
-    const int seg_T = pic_segment_target(s_off[256]);
-    for (int t = tid; t < 256; t += PIC_STEP_THREADS) {
+    const int seg_T = pic_segment_target(s_off[256], d.seg_num);
+    if (!SPARSE)
+    for (int t = tid; t < 256; t += NT) {
         const int c = d.cell_perm[(size_t)s * 256 + t];
         const int n = s_off[c + 1] - s_off[c];
         const int k = (n + seg_T - 1) / seg_T;
@@ -251,6 +374,34 @@ __global__ void __launch_bounds__(PIC_STEP_THREADS, 2) pic_step_kernel(const Pic
     const int n_items = s_nitems;
     constexpr int SX = 1, SY = G::JNX, SZ = G::JNX * G::JNY;
 
+    const int count = s_off[256];
+    if (SPARSE) {
+        // sparse supercell (a few particles per cell): register sums would be flushed almost once per
+        // particle, so take one thread per particle, coalesced, and deposit straight into the tile
+        for (int base = 0; base < count; base += NT) {
+            if (base + (tid & ~31) >= count) continue;       // warp-uniform
+            const int slot = base + tid;
+            const bool active = slot < count;
+            float4 P = make_float4(0.5f, 0.5f, 0.5f, 0.0f), M = make_float4(0.f, 0.f, 0.f, 0.f);   // ghost lane
+            size_t idx = 0;
+            if (active) {
+                idx = (size_t)tbl[slot >> 8] * PIC_FRAME + (slot & (PIC_FRAME - 1));
+                P = rec[2 * idx];
+                M = rec[2 * idx + 1];
+            }
+            const uint32_t bits = __float_as_uint(M.w);
+            const int lc = bits & 0xff, sp = (bits >> 16) & 0xff;
+            const int cx = lc & 7, cy = (lc >> 3) & 7, cz = lc >> 6;
+            float un[3], fn[3], x1[3];
+            int sh[3];
+            push_particle<O>(d, sF, cx, cy, cz, sp, P, M, un, fn, x1, sh);
+            const float f0[3] = {P.x, P.y, P.z};
+            deposit_direct<O, FIX>(d, sJ, sJhi, sJlo, fix_scale, f0, x1, d.q[sp] * P.w, lc);
+            if (active)
+                finish_particle(d, rec, idx, s, ssx, ssy, ssz, cx, cy, cz, sp, P, M, un, fn, sh, s_hist, &s_xn, s_xrec,
+                                s_xid, s_xdst);
+        }
+    } else
     for (;;) {   // a warp takes 32 work items at a time
     int ibase = 0;
     if (lane == 0) ibase = atomicAdd(&s_next, 32);
@@ -290,65 +441,11 @@ __global__ void __launch_bounds__(PIC_STEP_THREADS, 2) pic_step_kernel(const Pic
         }
         const int sp = (__float_as_uint(M.w) >> 16) & 0xff;
 
-        // ---- a2: gather at x^n
-        float E[3], B[3];
-        {
-            float wu[3][O + 1], ws[3][O + 1];
-            int bu[3], bs[3];
-            const float f[3] = {P.x, P.y, P.z};
-#pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                bu[a] = shape<O>(f[a], wu[a]);
-                bs[a] = shape<O>(f[a] - 0.5f, ws[a]);
-            }
-            const int ux_ = cx + bu[0] + G::FL, sx_ = cx + bs[0] + G::FL;
-            const int uy_ = (cy + bu[1] + G::FL) * G::FPX, sy_ = (cy + bs[1] + G::FL) * G::FPX;
-            const int uz_ = (cz + bu[2] + G::FL) * G::FPX * G::FNY, sz_ = (cz + bs[2] + G::FL) * G::FPX * G::FNY;
-            E[0] = gather1<O>(sF + 0 * G::FCOMP + sx_ + uy_ + uz_, ws[0], wu[1], wu[2]);
-            E[1] = gather1<O>(sF + 1 * G::FCOMP + ux_ + sy_ + uz_, wu[0], ws[1], wu[2]);
-            E[2] = gather1<O>(sF + 2 * G::FCOMP + ux_ + uy_ + sz_, wu[0], wu[1], ws[2]);
-            B[0] = gather1<O>(sF + 3 * G::FCOMP + ux_ + sy_ + sz_, wu[0], ws[1], ws[2]);
-            B[1] = gather1<O>(sF + 4 * G::FCOMP + sx_ + uy_ + sz_, ws[0], wu[1], ws[2]);
-            B[2] = gather1<O>(sF + 5 * G::FCOMP + sx_ + sy_ + uz_, ws[0], ws[1], wu[2]);
-        }
-
-        // ---- a3: Boris push and move (step 5)
-        const float h = d.h[sp];
-        const float umx = fmaf(h, E[0], M.x), umy = fmaf(h, E[1], M.y), umz = fmaf(h, E[2], M.z);
-        const float igm = rsqrtf(1.0f + umx * umx + umy * umy + umz * umz);
-        const float tx = h * B[0] * igm, ty = h * B[1] * igm, tz = h * B[2] * igm;
-        const float sfac = 2.0f / (1.0f + tx * tx + ty * ty + tz * tz);
-        const float upx = umx + (umy * tz - umz * ty);
-        const float upy = umy + (umz * tx - umx * tz);
-        const float upz = umz + (umx * ty - umy * tx);
-        const float sx2 = tx * sfac, sy2 = ty * sfac, sz2 = tz * sfac;
-        const float unx = fmaf(h, E[0], umx + (upy * sz2 - upz * sy2));
-        const float uny = fmaf(h, E[1], umy + (upz * sx2 - upx * sz2));
-        const float unz = fmaf(h, E[2], umz + (upx * sy2 - upy * sx2));
-        const float ig = rsqrtf(1.0f + unx * unx + uny * uny + unz * unz);
-        const float del[3] = {unx * ig * d.dtdx, uny * ig * d.dtdy, unz * ig * d.dtdz};
-
-        // new in-cell fraction and cell shift (reading S19)
-        const float f0[3] = {P.x, P.y, P.z};
-        float fn[3], x1[3];
+        float un[3], fn[3], x1[3];
         int sh[3];
-        bool far = false;
-#pragma unroll
-        for (int a = 0; a < 3; ++a) {
-            float fp = f0[a] + del[a];
-            float fl = floorf(fp);
-            float g = fp - fl;
-            int shift = (int)fl;
-            if (g >= 1.0f) {            // tiny negative fp: fp + 1 rounded up to 1
-                g = 0.0f;
-                shift += 1;
-            }
-            far |= (shift < -1) | (shift > 1);
-            fn[a] = g;
-            sh[a] = shift;
-            x1[a] = (float)shift + g;   // new position relative to the OLD cell's origin node
-        }
-        if (far) atomicOr(d.ctr + CTR_ERROR, PIC_DEV_MOVED_TOO_FAR);
+        push_particle<O>(d, sF, cx, cy, cz, sp, P, M, un, fn, x1, sh);
+        const float f0[3] = {P.x, P.y, P.z};
+
 
         // ---- a4: Esirkepov, accumulated in registers over the cell's window (nodes -1..2)
         {
@@ -383,40 +480,7 @@ __global__ void __launch_bounds__(PIC_STEP_THREADS, 2) pic_step_kernel(const Pic
             }
         }
 
-        // ---- a5: new cell, destination supercell, write back in place
-        int ncx = cx + sh[0], ncy = cy + sh[1], ncz = cz + sh[2];
-        const int dsx = (ncx < 0) ? -1 : (ncx >= PIC_SCX) ? 1 : 0;
-        const int dsy = (ncy < 0) ? -1 : (ncy >= PIC_SCY) ? 1 : 0;
-        const int dsz = (ncz < 0) ? -1 : (ncz >= PIC_SCZ) ? 1 : 0;
-        ncx -= dsx * PIC_SCX; ncy -= dsy * PIC_SCY; ncz -= dsz * PIC_SCZ;
-        const int nlc = ncx + PIC_SCX * (ncy + PIC_SCY * ncz);
-        const uint32_t nbits = pic_pack_bits(nlc, sp);
-        P.x = fn[0]; P.y = fn[1]; P.z = fn[2];
-        M.x = unx; M.y = uny; M.z = unz;
-        if ((dsx | dsy | dsz) == 0) {
-            M.w = __uint_as_float(nbits);
-            rec[2 * idx] = P;
-            rec[2 * idx + 1] = M;
-            atomicAdd(&s_hist[nlc], 1);
-        } else {
-            const int dst = wrapi(ssx + dsx, d.nsx) + d.nsx * (wrapi(ssy + dsy, d.nsy) + d.nsy * wrapi(ssz + dsz, d.nsz));
-            rec[2 * idx + 1] = make_float4(unx, uny, unz, __uint_as_float(nbits | PIC_LEFT_FLAG));   // hole
-            M.w = __uint_as_float(nbits);
-            const uint32_t id = d.pid[d.cur][idx];
-            const int k = atomicAdd(&s_xn, 1);
-            if (k < PIC_XSTAGE) {
-                s_xrec[2 * k] = P; s_xrec[2 * k + 1] = M; s_xid[k] = id; s_xdst[k] = dst;
-            } else {                      // staging full: append directly
-                const int xs = atomicAdd(d.ctr + CTR_EXCH, 1);
-                if (xs < d.x_cap) {
-                    d.x_rec[2 * (size_t)xs] = P; d.x_rec[2 * (size_t)xs + 1] = M; d.x_id[xs] = id; d.x_dst[xs] = dst;
-                } else {
-                    atomicOr(d.ctr + CTR_ERROR, PIC_DEV_EXCHANGE_OVERFLOW);
-                }
-            }
-            atomicAdd(d.cell_hist + (size_t)dst * 256 + nlc, 1);
-            atomicAdd(d.sc_incoming + dst, 1);
-        }
+        finish_particle(d, rec, idx, s, ssx, ssy, ssz, cx, cy, cz, sp, P, M, un, fn, sh, s_hist, &s_xn, s_xrec, s_xid, s_xdst);
     }
 
     // ---- a4: one flush of the segment's 3 x 48 partial sums into the shared tile (warp-synchronous)
@@ -439,7 +503,7 @@ __global__ void __launch_bounds__(PIC_STEP_THREADS, 2) pic_step_kernel(const Pic
     // ---- a4: queued out-of-window particles, one thread each
     {
         const int n_slow = min(s_slown, PIC_SLOWCAP);
-        for (int base = 0; base < n_slow; base += PIC_STEP_THREADS) {
+        for (int base = 0; base < n_slow; base += NT) {
             if (base + (tid & ~31) < n_slow) {          // warp-uniform
                 const int e = base + tid;
                 float f0[3] = {0.5f, 0.5f, 0.5f}, x1[3] = {0.5f, 0.5f, 0.5f}, qw = 0.0f;
@@ -459,7 +523,7 @@ __global__ void __launch_bounds__(PIC_STEP_THREADS, 2) pic_step_kernel(const Pic
     const int n_x = min(s_xn, PIC_XSTAGE);
     if (tid == 0 && n_x > 0) s_xbase = atomicAdd(d.ctr + CTR_EXCH, n_x);
     __syncthreads();
-    for (int k = tid; k < n_x; k += PIC_STEP_THREADS) {
+    for (int k = tid; k < n_x; k += NT) {
         const int xs = s_xbase + k;
         if (xs < d.x_cap) {
             d.x_rec[2 * (size_t)xs] = s_xrec[2 * k];
@@ -471,13 +535,13 @@ __global__ void __launch_bounds__(PIC_STEP_THREADS, 2) pic_step_kernel(const Pic
         }
     }
     // stayers per new cell (neighbours add their leavers to the same counters)
-    for (int t = tid; t < 256; t += PIC_STEP_THREADS)
+    for (int t = tid; t < 256; t += NT)
         if (s_hist[t] != 0) atomicAdd(d.cell_hist + (size_t)s * 256 + t, s_hist[t]);
 
     // ---- a4: flush the J tile once (periodic wrap on write)
     {
         const size_t ncell = (size_t)d.nx * d.ny * d.nz;
-        for (int e = tid; e < 3 * G::JCOMP; e += PIC_STEP_THREADS) {
+        for (int e = tid; e < 3 * G::JCOMP; e += NT) {
             int i = e % G::JNX;
             int r = e / G::JNX;
             int j = r % G::JNY;
@@ -583,6 +647,7 @@ __global__ void __launch_bounds__(PIC_FRAME) pic_sort_kernel(const PicDev d)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int s = blockIdx.x;
     const int n_scan = d.sc_tail[s];
+    if (n_scan == 0) return;       // empty and nothing arrived: ranges, count and histogram are already zero
     const int cnt = d.cell_hist[(size_t)s * 256 + tid];
     d.cell_hist[(size_t)s * 256 + tid] = 0;
     s_cnt[tid] = cnt;
@@ -610,7 +675,8 @@ __global__ void __launch_bounds__(PIC_FRAME) pic_sort_kernel(const PicDev d)
     }
     // work items of the next step: cell c is cut into k = ceil(n/T) segments of ~n/k particles; order
     // the cells by decreasing segment length (ties by index) and publish the first item of each
-    const int seg_T = pic_segment_target(total);
+    if (total >= PIC_DIRECT_BELOW) {   // block-uniform; the per-particle path needs no work items
+    const int seg_T = pic_segment_target(total, d.seg_num);
     const int k = (cnt + seg_T - 1) / seg_T;
     const int seglen = k ? (cnt + k - 1) / k : 0;
     __syncthreads();               // s_cnt is complete; reuse it for the keys
@@ -643,6 +709,7 @@ __global__ void __launch_bounds__(PIC_FRAME) pic_sort_kernel(const PicDev d)
             if (w < warp) kb += s_wsum[w];
         d.cell_kbase[(size_t)s * 256 + tid] = (unsigned short)min(kb + ki - kk, 65535);
     }
+    }
     __syncthreads();
     if (total > n_scan) {          // histogram and records disagree: never write out of bounds
         if (tid == 0) atomicOr(d.ctr + CTR_ERROR, PIC_DEV_SORT_MISMATCH);
@@ -674,18 +741,28 @@ __global__ void __launch_bounds__(PIC_FRAME) pic_sort_kernel(const PicDev d)
 
 }  // namespace
 
-template <int O, bool TMA, bool FIX>
-static cudaError_t launch_step_variant(const PicDev& d, const CUtensorMap& map, cudaStream_t st)
+template <int O, bool TMA, bool FIX, bool SPARSE>
+static cudaError_t launch_step_one(const PicDev& d, const CUtensorMap& map, cudaStream_t st)
 {
     static bool configured = false;     // opt in to > 48 KB of dynamic shared memory once
-    constexpr int bytes = StepSmem<O, FIX>::TOTAL;
+    constexpr int bytes = SPARSE ? StepSmem<O, FIX>::OFF_SLOW : StepSmem<O, FIX>::TOTAL;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(pic_step_kernel<O, TMA, FIX>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+        cudaError_t e = cudaFuncSetAttribute(pic_step_kernel<O, TMA, FIX, SPARSE>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    pic_step_kernel<O, TMA, FIX><<<d.nsc, PIC_STEP_THREADS, bytes, st>>>(d, map);
+    pic_step_kernel<O, TMA, FIX, SPARSE><<<d.nsc, SPARSE ? 256 : PIC_STEP_THREADS, bytes, st>>>(d, map);
     return cudaGetLastError();
+}
+
+template <int O, bool TMA, bool FIX>
+static cudaError_t launch_step_variant(const PicDev& d, const CUtensorMap& map, cudaStream_t st, int64_t* launches)
+{
+    cudaError_t e = launch_step_one<O, TMA, FIX, false>(d, map, st);
+    if (e == cudaSuccess) e = launch_step_one<O, TMA, FIX, true>(d, map, st);
+    *launches += 2;
+    return e;
 }
 
 cudaError_t pic_launch_step(const PicDev& d, int order, bool use_tma, bool fixed_point, const void* tmap,
@@ -695,17 +772,16 @@ cudaError_t pic_launch_step(const PicDev& d, int order, bool use_tma, bool fixed
     if (use_tma) memcpy(&map, tmap, sizeof map); else memset(&map, 0, sizeof map);
     cudaError_t e;
 #define PIC_GO(O)                                                                               \
-    e = use_tma ? (fixed_point ? launch_step_variant<O, true, true>(d, map, st)                 \
-                               : launch_step_variant<O, true, false>(d, map, st))               \
-                : (fixed_point ? launch_step_variant<O, false, true>(d, map, st)                \
-                               : launch_step_variant<O, false, false>(d, map, st))
+    e = use_tma ? (fixed_point ? launch_step_variant<O, true, true>(d, map, st, launches)                 \
+                               : launch_step_variant<O, true, false>(d, map, st, launches))               \
+                : (fixed_point ? launch_step_variant<O, false, true>(d, map, st, launches)                \
+                               : launch_step_variant<O, false, false>(d, map, st, launches))
     switch (order) {
         case 1: PIC_GO(1); break;
         case 2: PIC_GO(2); break;
         default: PIC_GO(3); break;
     }
 #undef PIC_GO
-    ++*launches;
     return e;
 }
 
