@@ -58,7 +58,7 @@ extern "C" {
 #define PIC_DEV_TABLE_POOL_EXHAUSTED   4
 #define PIC_DEV_MOVED_TOO_FAR          8
 #define PIC_DEV_TMA_TIMEOUT           16
-#define PIC_DEV_SLOW_QUEUE_FULL       32   /* > 768 particles of one supercell left their cell's 4-node window */
+#define PIC_DEV_OVERFLOW_QUEUE_FULL   32   /* out-of-window particles exceeded the global overflow queue */
 #define PIC_DEV_SORT_MISMATCH         64   /* internal: cell histogram and records disagree */
 
 typedef struct pic_ctx pic_ctx;   /* opaque, host-side */

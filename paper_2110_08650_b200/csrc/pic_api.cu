@@ -42,7 +42,7 @@ namespace {
 
 struct Layout {
     uint64_t rec0, rec1, pid0, pid1, tbl_pool, tbl_off, tbl_cap, sc_nframes, sc_count, sc_tail, sc_incoming,
-        cell_off, cell_hist, cell_perm, cell_kbase, x_rec, x_id, x_dst, ctr, ctr64, F, Fpad, J, J64, sc_offset, total;
+        cell_off, cell_hist, cell_perm, cell_kbase, x_rec, x_id, x_dst, ovf, ctr, ctr64, F, Fpad, J, J64, sc_offset, total;
     int n_frames, tbl_pool_size, x_cap, nsc;
 };
 
@@ -85,6 +85,7 @@ int compute_layout(const int32_t grid[3], const int32_t sc[3], int order, int64_
     L->x_rec = take(xcap * 32);
     L->x_id = take(xcap * 4);
     L->x_dst = take(xcap * 4);
+    L->ovf = take(xcap * 32);
     L->ctr = take(CTR_N * 4);
     L->ctr64 = take(CTR64_N * 8);
     L->F = take(6 * ncell * 4);
@@ -288,7 +289,7 @@ int check_device(pic_ctx* c)
     if (e != cudaSuccess) return cuda_fail(c, e, "reading the device error word");
     if (err) {
         char buf[160];
-        snprintf(buf, sizeof buf, "device fault word 0x%x (1 frame pool, 2 exchange buffer, 4 table pool, 8 moved >= 1 cell, 16 TMA timeout)", err);
+        snprintf(buf, sizeof buf, "device fault word 0x%x (1 frame pool, 2 exchange buffer, 4 table pool, 8 moved >= 1 cell, 16 TMA timeout, 32 overflow queue, 64 sort mismatch)", err);
         return fail(c, PIC_EDEVICE, buf);
     }
     return PIC_OK;
@@ -400,6 +401,7 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     d.cell_perm = (unsigned char*)(w + L.cell_perm);
     d.cell_kbase = (unsigned short*)(w + L.cell_kbase);
     d.x_rec = (float4*)(w + L.x_rec);
+    d.ovf = (float4*)(w + L.ovf); d.ovf_cap = L.x_cap;
     d.x_id = (uint32_t*)(w + L.x_id); d.x_dst = (int*)(w + L.x_dst); d.x_cap = L.x_cap;
     d.ctr = (int*)(w + L.ctr); d.ctr64 = (unsigned long long*)(w + L.ctr64);
     d.F = (const float*)(w + L.F); d.Fpad = (const float*)(w + L.Fpad); d.J = (float*)(w + L.J); d.J64 = (long long*)(w + L.J64);
@@ -488,6 +490,7 @@ static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
         cudaError_t e = c->fixed_point ? cudaMemsetAsync(d.J64, 0, 3 * ncell * sizeof(long long), st)   // S16
                                        : cudaMemsetAsync(d.J, 0, 3 * ncell * sizeof(float), st);
         if (e == cudaSuccess) e = cudaMemsetAsync(d.ctr + CTR_EXCH, 0, sizeof(int), st);
+        if (e == cudaSuccess) e = cudaMemsetAsync(d.ctr + CTR_OVF, 0, sizeof(int), st);
         cudaEvent_t ev0 = nullptr, ev1 = nullptr;
         if (e == cudaSuccess && c->timing) {
             e = cudaEventCreate(&ev0);
@@ -500,6 +503,7 @@ static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
             c->events.push_back(ev0);
             c->events.push_back(ev1);
         }
+        if (e == cudaSuccess) e = pic_launch_overflow(d, c->order, c->fixed_point, st, &c->launches);
         if (e == cudaSuccess && c->fixed_point) e = pic_launch_convert(d, st, &c->launches);
         if (e == cudaSuccess) e = pic_launch_prepare(d, st, &c->launches);
         if (e == cudaSuccess) e = pic_launch_scatter(d, st, &c->launches);

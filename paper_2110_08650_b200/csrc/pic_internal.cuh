@@ -31,7 +31,9 @@ enum {
     CTR_ERROR = 3,        // sticky error word (PIC_DEV_* bits)
     CTR_LEAVERS_LAST = 4,
     CTR_MAX_COUNT = 5,
-    CTR_WMAX_BITS = 6,    // bits of max |weight| loaded so far (non-negative floats order like ints)
+    CTR_WMAX_BITS = 6,
+    CTR_OVF = 7,          // entries in the overflow queue of out-of-window particles (this step)
+       // bits of max |weight| loaded so far (non-negative floats order like ints)
     CTR_N = 16
 };
 // 64-bit counters in PicDev::ctr64
@@ -69,6 +71,8 @@ struct PicDev {
     uint32_t* x_id;
     int* x_dst;
     int x_cap;
+    float4* ovf;                 // overflow queue of out-of-window particles, 2 float4 per entry
+    int ovf_cap;
     // counters
     int* ctr;
     unsigned long long* ctr64;
@@ -105,6 +109,7 @@ __host__ __device__ inline uint32_t pic_pack_bits(int local_cell, int species)
 // launchers implemented in pic_step.cu
 cudaError_t pic_launch_step(const PicDev& d, int order, bool use_tma, bool fixed_point, const void* tmap,
                             cudaStream_t st, int64_t* launches);
+cudaError_t pic_launch_overflow(const PicDev& d, int order, bool fixed_point, cudaStream_t st, int64_t* launches);
 cudaError_t pic_launch_convert(const PicDev& d, cudaStream_t st, int64_t* launches);
 cudaError_t pic_launch_prepare(const PicDev& d, cudaStream_t st, int64_t* launches);
 cudaError_t pic_launch_scatter(const PicDev& d, cudaStream_t st, int64_t* launches);

@@ -119,6 +119,7 @@ __device__ __forceinline__ void deposit_direct(const PicDev& d, float* sJ, int* 
                      wide[2], wide[0], wide[1], lwide[2], DS[2], S0[0], DS[0], S0[1], DS[1]);
 }
 
+
 // register accumulation of one component over the cell's window:
 // A[i][b][c] += fac * (sum_{i'<=i} DS_a(i')) * bracket(b,c),  i = nodes -1,0,1 of the flow axis
 __device__ __forceinline__ void accumulate1(float (&A)[3][4][4], float fac, const float (&DSa)[4],
@@ -474,8 +475,14 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
                     q[0] = f0[0]; q[1] = f0[1]; q[2] = f0[2];
                     q[3] = x1[0]; q[4] = x1[1]; q[5] = x1[2];
                     q[6] = qw; q[7] = __int_as_float(lc);
-                } else {
-                    atomicOr(d.ctr + CTR_ERROR, PIC_DEV_SLOW_QUEUE_FULL);
+                } else {            // queue full: hand the particle to pic_overflow_kernel
+                    const int k2 = atomicAdd(d.ctr + CTR_OVF, 1);
+                    if (k2 < d.ovf_cap) {
+                        d.ovf[2 * (size_t)k2] = make_float4(f0[0], f0[1], f0[2], qw);
+                        d.ovf[2 * (size_t)k2 + 1] = make_float4(x1[0], x1[1], x1[2], __int_as_float(lc | (s << 8)));
+                    } else {
+                        atomicOr(d.ctr + CTR_ERROR, PIC_DEV_OVERFLOW_QUEUE_FULL);
+                    }
                 }
             }
         }
@@ -559,6 +566,65 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
                 const float v = sJ[e];
                 if (v != 0.0f) atomicAdd(d.J + g, v);
             }
+        }
+    }
+}
+
+// Out-of-window particles that did not fit a CTA's shared-memory queue: one thread per particle,
+// Esirkepov straight into the global accumulators (rare: needs > 768 such particles in one supercell).
+template <int O, bool FIX>
+__global__ void pic_overflow_kernel(const PicDev d)
+{
+    const int n = min(d.ctr[CTR_OVF], d.ovf_cap);
+    const size_t ncell = (size_t)d.nx * d.ny * d.nz;
+    const float jf[3] = {d.jfx, d.jfy, d.jfz};
+    const int dims[3] = {d.nx, d.ny, d.nz};
+    const size_t stride[3] = {1, (size_t)d.nx, (size_t)d.nx * d.ny};
+    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
+        const float4 A = d.ovf[2 * (size_t)e], Bq = d.ovf[2 * (size_t)e + 1];
+        const float f0[3] = {A.x, A.y, A.z}, x1[3] = {Bq.x, Bq.y, Bq.z};
+        const float qw = A.w;
+        const int code = __float_as_int(Bq.w);
+        const int lc = code & 255, s = code >> 8;
+        const int cell[3] = {(s % d.nsx) * PIC_SCX + (lc & 7), ((s / d.nsx) % d.nsy) * PIC_SCY + ((lc >> 3) & 7),
+                             (s / (d.nsx * d.nsy)) * PIC_SCZ + (lc >> 6)};
+        float S0[3][O + 2], DS[3][O + 2];
+        int lo[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            float w0[O + 1], w1[O + 1], s1[O + 2];
+            const int b0 = shape<O>(f0[a], w0), b1 = shape<O>(x1[a], w1);
+            lo[a] = min(b0, b1);
+            to_window<O>(w0, b0 - lo[a], S0[a]);
+            to_window<O>(w1, b1 - lo[a], s1);
+#pragma unroll
+            for (int t = 0; t < O + 2; ++t) DS[a][t] = s1[t] - S0[a][t];
+        }
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const int b = (a + 1) % 3, c = (a + 2) % 3;
+            const float scale = FIX ? fix_scale_of(d, jf[a]) : 1.0f;
+            const float fac = -qw * jf[a] * scale;
+            for (int tc = 0; tc < O + 2; ++tc)
+                for (int tb = 0; tb < O + 2; ++tb) {
+                    const float br = fac * (S0[b][tb] * S0[c][tc] + 0.5f * DS[b][tb] * S0[c][tc] +
+                                            0.5f * S0[b][tb] * DS[c][tc] + (1.0f / 3.0f) * DS[b][tb] * DS[c][tc]);
+                    float acc = 0.0f;
+                    for (int ta = 0; ta < O + 1; ++ta) {
+                        acc = fmaf(DS[a][ta], br, acc);
+                        if (acc == 0.0f) continue;
+                        int idx[3];
+                        idx[a] = cell[a] + lo[a] + ta; idx[b] = cell[b] + lo[b] + tb; idx[c] = cell[c] + lo[c] + tc;
+                        size_t g = a * ncell;
+#pragma unroll
+                        for (int x = 0; x < 3; ++x) g += stride[x] * (size_t)wrapi(idx[x], dims[x]);
+                        if (FIX)
+                            atomicAdd(reinterpret_cast<unsigned long long*>(d.J64) + g,
+                                      (unsigned long long)__double2ll_rn((double)acc * (double)(1 << PIC_FIX_LO_BITS)));
+                        else
+                            atomicAdd(d.J + g, acc);
+                    }
+                }
         }
     }
 }
@@ -783,6 +849,21 @@ cudaError_t pic_launch_step(const PicDev& d, int order, bool use_tma, bool fixed
     }
 #undef PIC_GO
     return e;
+}
+
+cudaError_t pic_launch_overflow(const PicDev& d, int order, bool fixed_point, cudaStream_t st, int64_t* launches)
+{
+    const dim3 g(148 * 2), b(128);
+    switch (order * 2 + (fixed_point ? 1 : 0)) {
+        case 2: pic_overflow_kernel<1, false><<<g, b, 0, st>>>(d); break;
+        case 3: pic_overflow_kernel<1, true><<<g, b, 0, st>>>(d); break;
+        case 4: pic_overflow_kernel<2, false><<<g, b, 0, st>>>(d); break;
+        case 5: pic_overflow_kernel<2, true><<<g, b, 0, st>>>(d); break;
+        case 6: pic_overflow_kernel<3, false><<<g, b, 0, st>>>(d); break;
+        default: pic_overflow_kernel<3, true><<<g, b, 0, st>>>(d); break;
+    }
+    ++*launches;
+    return cudaGetLastError();
 }
 
 cudaError_t pic_launch_convert(const PicDev& d, cudaStream_t st, int64_t* launches)

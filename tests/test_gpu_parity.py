@@ -101,6 +101,25 @@ def test_gpu_continuity(name):
     pic.destroy()
 
 
+@pytest.mark.parametrize("order", (1, 2, 3))
+def test_fast_particles_leave_the_register_window(order):
+    """c*dt = 0.9 cell and relativistic momenta: most particles move more than half a cell, leave their
+    cell's 4-node register window, fill the shared-memory queue (768 per supercell) and spill into the
+    on-the-spot deposit.  Same tolerances."""
+    wl = W.CONFIGS["thermal_128"].scaled((16, 16, 8), shape_order=order, ppc=16, u_th=1.0, dt=0.9)
+    parts, fields = W.make_particles(wl), W.make_fields(wl)
+    orc = PP.oracle_for(wl, parts, fields)
+    pic = PP.gpu_for(wl, parts, fields)
+    assert orc.step(2) == 0
+    pic.step(2)
+    rep = PP.compare(wl, orc, pic, 2, 1.0)
+    print(f"\n[fast particles order {order}] {rep}")
+    assert rep.max_dx <= 2 * PP.TOL_X and rep.max_du_rel <= 2 * PP.TOL_U and rep.j_err_rel <= 2 * PP.TOL_J1
+    assert rep.n_member_mismatch == 0 and rep.counts_equal_outside_band
+    assert pic.get_stats()["error"] == 0
+    pic.destroy()
+
+
 def test_species_table_and_anisotropic_cells():
     """Positive charge / heavier species and dx != dy != dz go through the same kernels."""
     wl = W.CONFIGS["khi"].scaled((16, 24, 8), cell=(1.0, 0.8, 1.25), dt=0.4)
