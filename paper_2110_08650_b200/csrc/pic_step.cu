@@ -133,13 +133,17 @@ __device__ __forceinline__ void accumulate1(float (&A)[3][4][4], float fac, cons
     for (int c = 0; c < 4; ++c) {
         const float c0 = S0c[c] + 0.5f * DSc[c];
         const float c1 = 0.5f * S0c[c] + (1.0f / 3.0f) * DSc[c];
+        float br[4];
 #pragma unroll
-        for (int b = 0; b < 4; ++b) {
-            const float br = fmaf(S0b[b], c0, DSb[b] * c1);
-            A[0][b][c] = fmaf(p0, br, A[0][b][c]);
-            A[1][b][c] = fmaf(p1, br, A[1][b][c]);
-            A[2][b][c] = fmaf(p2, br, A[2][b][c]);
+        for (int b = 0; b < 4; b += 2) {
+            br[b] = DSb[b] * c1;
+            br[b + 1] = DSb[b + 1] * c1;
+            ffma2(br[b], br[b + 1], S0b[b], S0b[b + 1], c0, c0);
         }
+#pragma unroll
+        for (int b = 0; b < 4; ++b) ffma2(A[0][b][c], A[1][b][c], p0, p1, br[b], br[b]);
+#pragma unroll
+        for (int b = 0; b < 4; b += 2) ffma2(A[2][b][c], A[2][b + 1][c], br[b], br[b + 1], p2, p2);
     }
 }
 
