@@ -57,7 +57,7 @@ int compute_layout(const int32_t grid[3], const int32_t sc[3], int order, int64_
         if (grid[a] <= 0 || grid[a] % sc[a] != 0) return PIC_EINVAL;
     const uint64_t nsc = (uint64_t)(grid[0] / sc[0]) * (grid[1] / sc[1]) * (grid[2] / sc[2]);
     const uint64_t ncell = (uint64_t)grid[0] * grid[1] * grid[2];
-    if (nsc > (1u << 30) || (uint64_t)maxp > (1ull << 32) - 1) return PIC_EINVAL;
+    if (nsc > (1u << 22) || (uint64_t)maxp > (1ull << 32) - 1) return PIC_EINVAL;   // supercell index is packed into 23 bits
     // every supercell may hold one partly filled frame; 1/8 head-room for density drift
     const uint64_t n_frames = (uint64_t)maxp / PIC_FRAME + (uint64_t)maxp / (8 * PIC_FRAME) + 2 * nsc + 64;
     const uint64_t slots = n_frames * PIC_FRAME;

@@ -790,22 +790,41 @@ __global__ void __launch_bounds__(PIC_FRAME) pic_sort_kernel(const PicDev d)
     float4* dst = d.rec[d.cur ^ 1];
     const uint32_t* sid = d.pid[d.cur];
     uint32_t* did = d.pid[d.cur ^ 1];
-    for (int slot = tid; slot < n_scan; slot += PIC_FRAME) {
-        const size_t i = (size_t)tbl[slot >> 8] * PIC_FRAME + (slot & (PIC_FRAME - 1));
-        const float4 M = src[2 * i + 1];
-        const uint32_t bits = __float_as_uint(M.w);
-        if (bits & PIC_LEFT_FLAG) continue;
-        const float4 P = src[2 * i];
-        const int c = bits & 0xff;
-        const int r = atomicAdd(&s_cur[c], 1);
-        if (r >= total) {
-            atomicOr(d.ctr + CTR_ERROR, PIC_DEV_SORT_MISMATCH);
-            continue;
+    // four slots per thread and iteration: all loads are issued before the first use
+    constexpr int U = 4;
+    for (int base = 0; base < n_scan; base += U * PIC_FRAME) {
+        size_t i[U];
+        float4 P[U], M[U];
+        uint32_t id[U];
+        bool ok[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int slot = base + u * PIC_FRAME + tid;
+            ok[u] = slot < n_scan;
+            i[u] = ok[u] ? (size_t)tbl[slot >> 8] * PIC_FRAME + (slot & (PIC_FRAME - 1)) : 0;
         }
-        const size_t o = (size_t)tbl[r >> 8] * PIC_FRAME + (r & (PIC_FRAME - 1));
-        dst[2 * o] = P;
-        dst[2 * o + 1] = M;
-        did[o] = sid[i];
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+            if (ok[u]) {
+                P[u] = src[2 * i[u]];
+                M[u] = src[2 * i[u] + 1];
+                id[u] = sid[i[u]];
+            }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            if (!ok[u]) continue;
+            const uint32_t bits = __float_as_uint(M[u].w);
+            if (bits & PIC_LEFT_FLAG) continue;
+            const int r = atomicAdd(&s_cur[bits & 0xff], 1);
+            if (r >= total) {
+                atomicOr(d.ctr + CTR_ERROR, PIC_DEV_SORT_MISMATCH);
+                continue;
+            }
+            const size_t o = (size_t)tbl[r >> 8] * PIC_FRAME + (r & (PIC_FRAME - 1));
+            dst[2 * o] = P[u];
+            dst[2 * o + 1] = M[u];
+            did[o] = id[u];
+        }
     }
 }
 
