@@ -78,7 +78,7 @@ CONFIGS: Dict[str, Workload] = {
     # configs[2]
     "lwfa": Workload("lwfa", (256, 1024, 256), 2, 2, 2, 50, u_th=0.0, fields="laser",
                      layout="slab_ramp",
-                     laser=dict(a0=2.0, w0=32.0, w_y=16.0, wavelength=16.0, y0_frac=0.125)),
+                     laser=dict(a0=2.0, w0=32.0, w_y=16.0, wavelength=16.0, y0_frac=0.375)),
     # configs[3] (+ hot-spot variant)
     "khi": Workload("khi", (192, 192, 192), 2, 9, 3, 100, u_th=0.01, fields="modes",
                     n_modes=8, amplitude=0.01, layout="two_stream", drift_beta=0.2),
@@ -131,7 +131,8 @@ def make_fields(wl: Workload, device="cpu") -> torch.Tensor:
             out[c] = (acc * (wl.amplitude / M)).to(torch.float32)
         return out
     if wl.fields == "laser":
-        # S13: E_x = a0 exp(-((y-y0)/w_y)^2 - ((x-xc)^2+(z-zc)^2)/w0^2) cos(k (y-y0)), B_z = E_x,
+        # S13 (y0: DESIGN.md reading D6 — inside the plasma, the static pulse would otherwise touch no particle):
+        # E_x = a0 exp(-((y-y0)/w_y)^2 - ((x-xc)^2+(z-zc)^2)/w0^2) cos(k (y-y0)), B_z = E_x,
         # each evaluated at its own Yee location; all other components 0.
         L = wl.laser
         xc, zc = nx / 2.0, nz / 2.0
