@@ -91,11 +91,25 @@ def _fullsize(name, u_scale, per_chunk_sample=1500, box_lo=(40, 40, 40)):
           f"membership mismatches={mism} (near-face {int(near.sum())}); J sub-box from {box['x'].numel()} particles: "
           f"err/max|J|={j_err:.3e}; leavers={st['leavers_last']} max_count={st['max_count']}")
     assert worst_x <= PP.TOL_X and worst_u <= PP.TOL_U and mism == 0 and j_err <= PP.TOL_J1
+    # ---- tier T3: nine more steps, then the invariants that hold at any size
+    del P, ids, order
+    pic.step(9)
+    pic.sync()
+    st = pic.get_stats()
+    assert st["error"] == 0 and st["steps"] == 10
+    assert int(pic.get_counts().sum()) == n
+    assert PP.gpu_membership_consistent(wl, pic)
+    ids = pic.get_particles()["id"].to(torch.int64) & 0xFFFFFFFF
+    assert torch.equal(torch.sort(ids).values, torch.arange(n, device=dev))
     pic.destroy()
 
 
 def test_config2_thermal_128_full_size():
     _fullsize("thermal_128", 0.05)
+
+
+def test_config4_khi_full_size():
+    _fullsize("khi", 0.01, per_chunk_sample=800)
 
 
 def test_config4_khi_hotspot_full_size():
