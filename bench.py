@@ -233,6 +233,8 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     wl = W.CONFIGS[args.workload]
+    if args.grid:      # reduced-grid copy of the workload (experiments only; the default is the full config)
+        wl = wl.scaled(tuple(int(v) for v in args.grid.split(",")))
     n = W.n_particles(wl)
     K, Wm = args.steps, max(args.warmup, 3)
     ws = torch.empty(workspace_bytes(wl.grid, wl.supercell, wl.shape_order, n) + 256, dtype=torch.uint8, device=dev)
@@ -325,6 +327,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--workload", default="thermal_128")
+    ap.add_argument("--grid", default="", help="nx,ny,nz: run a reduced-grid copy of the workload")
     ap.add_argument("--tma", type=int, default=1)
     ap.add_argument("--deposit", type=int, default=1, help="1 fixed-point integer atomics, 0 float CAS atomics")
     ap.add_argument("--segment", type=int, default=3, help="work-item length in quarters of the mean cell population")
