@@ -283,13 +283,15 @@ def run_ours(args):
         peak, peak_src = measured_peaks()
         b_alg = algorithmic_bytes_per_particle_step(wl, n)
         achieved = b_alg * n / (kernel_ms_avg * 1e-3) / 1e9
-        traffic = None
+        traffic, ncu_extra = None, {}
         tpath = os.path.join(ROOT, "profiles", "step_kernel_traffic.json")
         if os.path.exists(tpath):
             with open(tpath) as f:
                 tj = json.load(f)
             if tj.get("workload") == wl.name:
                 traffic = tj.get("dram_bytes_per_launch")
+                ncu_extra = {k: tj[k] for k in ("warp_instructions_per_launch", "shared_pipe_busy_pct",
+                                                "issue_slots_busy_pct") if k in tj}
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
             n_s = {1: 4_000_000, 2: 2_400_000, 3: 1_600_000}[wl.shape_order]
@@ -311,7 +313,10 @@ def run_ours(args):
                          "traffic": traffic, "peak_source": peak_src, "kernel": "pic_step_kernel",
                          "kernel_ms": kernel_ms_avg, "bytes_per_particle_step": b_alg,
                          "frac_of_8000_GBps": achieved / 8000.0,
-                         "kernel_share_of_step": kernel_ms_avg / (ms_max / K)},
+                         "kernel_share_of_step": kernel_ms_avg / (ms_max / K),
+                         "binding_resource": "shared-memory pipe, then instruction issue (ncu: profiles/README.md); "
+                                             "HBM is the bound the metric names, not the one the kernel hits",
+                         "ncu": ncu_extra},
             "cpu_baseline": cpu,
             "e2e": e2e,
             "gpu_launches": launches, "clocks": clocks,
