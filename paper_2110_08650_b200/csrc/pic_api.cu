@@ -41,7 +41,7 @@ static std::string g_create_error;
 namespace {
 
 struct Layout {
-    uint64_t rec0, rec1, pid0, pid1, tbl_pool, tbl_off, tbl_cap, sc_nframes, sc_count, sc_tail, sc_incoming,
+    uint64_t rec0, rec1, pid0, pid1, free_stack, tbl_pool, tbl_off, tbl_cap, sc_nframes, sc_count, sc_tail, sc_incoming,
         cell_off, cell_hist, cell_perm, cell_kbase, x_rec, x_id, x_dst, ovf, ctr, ctr64, F, Fpad, J, J64, sc_offset, total;
     int n_frames, tbl_pool_size, x_cap, nsc;
 };
@@ -71,6 +71,7 @@ int compute_layout(const int32_t grid[3], const int32_t sc[3], int order, int64_
     L->rec1 = take(slots * 32);
     L->pid0 = take(slots * 4);
     L->pid1 = take(slots * 4);
+    L->free_stack = take(n_frames * 4);
     L->tbl_pool = take(tblp * 4);
     L->tbl_off = take(nsc * 4);
     L->tbl_cap = take(nsc * 4);
@@ -170,6 +171,7 @@ __global__ void pic_load_count_kernel(const PicDev d, const LoadArgs a)
 
 __global__ void pic_load_scatter_kernel(const PicDev d, const LoadArgs a)
 {
+    if (blockIdx.x == 0 && threadIdx.x == 0 && d.ctr[CTR_FREE_TOP] < 0) d.ctr[CTR_FREE_TOP] = 0;   // see pic_prepare_kernel
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < a.n;
          i += (long long)gridDim.x * blockDim.x) {
         float4 P;
@@ -398,6 +400,7 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     d.cur = 0;
     d.seg_num = 3;
     d.n_frames = L.n_frames;
+    d.free_stack = (int*)(w + L.free_stack);
     d.tbl_pool = (int*)(w + L.tbl_pool); d.tbl_pool_size = L.tbl_pool_size;
     d.tbl_off = (int*)(w + L.tbl_off); d.tbl_cap = (int*)(w + L.tbl_cap);
     d.sc_nframes = (int*)(w + L.sc_nframes); d.sc_count = (int*)(w + L.sc_count);

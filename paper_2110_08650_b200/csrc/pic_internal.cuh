@@ -32,7 +32,8 @@ enum {
     CTR_LEAVERS_LAST = 4,
     CTR_MAX_COUNT = 5,
     CTR_WMAX_BITS = 6,
-    CTR_OVF = 7,          // entries in the overflow queue of out-of-window particles (this step)
+    CTR_OVF = 7,
+    CTR_FREE_TOP = 8,     // entries on the stack of returned frames (may dip below 0 while prepare pops)          // entries in the overflow queue of out-of-window particles (this step)
        // bits of max |weight| loaded so far (non-negative floats order like ints)
     CTR_N = 16
 };
@@ -54,6 +55,7 @@ struct PicDev {
     int cur;                     // pool holding the current state
     int seg_num;                 // work-item length target in quarters of the mean cell population (2..16)
     int n_frames;
+    int* free_stack;             // [n_frames] frames returned by shrinking supercells
     int* tbl_pool;
     int tbl_pool_size;
     int* tbl_off;                // [nsc]

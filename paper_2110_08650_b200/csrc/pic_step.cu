@@ -669,13 +669,23 @@ __global__ void pic_prepare_kernel(const PicDev d)
             d.tbl_off[s] = off = noff;
             d.tbl_cap[s] = ncap;
         }
-        const int nnew = need - have;
-        const int f0 = atomicAdd(d.ctr + CTR_POOL_TOP, nnew);
-        if (f0 + nnew > d.n_frames) {
-            atomicOr(d.ctr + CTR_ERROR, PIC_DEV_FRAME_POOL_EXHAUSTED);
-            return;
+        // returned frames first (this kernel only pops, the sort kernel only pushes; the counter may
+        // dip below zero here and is clamped by the next kernel), then fresh ones from the pool
+        for (int i = have; i < need; ++i) {
+            int f;
+            const int t = atomicSub(d.ctr + CTR_FREE_TOP, 1);
+            if (t > 0) {
+                f = d.free_stack[t - 1];
+            } else {
+                f = atomicAdd(d.ctr + CTR_POOL_TOP, 1);
+                if (f >= d.n_frames) {
+                    atomicOr(d.ctr + CTR_ERROR, PIC_DEV_FRAME_POOL_EXHAUSTED);
+                    d.sc_nframes[s] = i;
+                    return;
+                }
+            }
+            d.tbl_pool[off + i] = f;
         }
-        for (int i = 0; i < nnew; ++i) d.tbl_pool[off + have + i] = f0 + i;
         d.sc_nframes[s] = need;
     }
     d.sc_tail[s] = count;
@@ -688,6 +698,7 @@ __global__ void pic_scatter_kernel(const PicDev d)
 {
     const int n = min(d.ctr[CTR_EXCH], d.x_cap);
     if (blockIdx.x == 0 && threadIdx.x == 0) {
+        if (d.ctr[CTR_FREE_TOP] < 0) d.ctr[CTR_FREE_TOP] = 0;      // see pic_prepare_kernel
         d.ctr[CTR_LEAVERS_LAST] = n;
         atomicAdd(d.ctr64 + CTR64_LEAVERS_CUM, (unsigned long long)n);
     }
@@ -824,6 +835,17 @@ __global__ void __launch_bounds__(PIC_FRAME) pic_sort_kernel(const PicDev d)
             dst[2 * o] = P[u];
             dst[2 * o + 1] = M[u];
             did[o] = id[u];
+        }
+    }
+    // a supercell that shrank returns the frames it no longer needs (one spare is kept); they are
+    // free in both pools and are handed out again by the next pic_prepare_kernel
+    __syncthreads();
+    if (tid == 0) {
+        const int keep = (total + PIC_FRAME - 1) / PIC_FRAME + 1, have = d.sc_nframes[s];
+        if (have > keep) {
+            const int at = atomicAdd(d.ctr + CTR_FREE_TOP, have - keep);
+            for (int i = keep; i < have; ++i) d.free_stack[at + i - keep] = tbl[i];
+            d.sc_nframes[s] = keep;
         }
     }
 }

@@ -120,6 +120,30 @@ def test_fast_particles_leave_the_register_window(order):
     pic.destroy()
 
 
+def test_long_run_with_bunching_reuses_frames():
+    """Static fields make the plasma bunch (max supercell population grows severalfold); supercells that
+    shrink must return their frames, or the pool (sized for 9/8 of the particles) runs dry."""
+    wl = W.CONFIGS["thermal_128"].scaled((32, 32, 32), amplitude=0.04)
+    parts, fields = W.make_particles(wl), W.make_fields(wl)
+    pic = PP.gpu_for(wl, parts, fields)
+    first = None
+    for _ in range(6):
+        pic.step(25)
+        st = pic.get_stats()
+        assert st["error"] == 0 and st["particles"] == parts.n
+        first = first or st
+    assert st["max_count"] > 1.5 * 4096, (first, st)      # the densest supercell grew well beyond the mean
+    assert st["frames_used"] <= st["frames_pool"]
+    assert PP.gpu_membership_consistent(wl, pic)
+    assert int(pic.get_counts().sum()) == parts.n
+    ids = pic.get_particles()["id"].to(torch.int64) & 0xFFFFFFFF
+    assert torch.equal(torch.sort(ids).values, torch.arange(parts.n, device=ids.device))
+    res = PP.gpu_continuity(wl, pic, [-1.0] * 16)
+    print(f"\n[long run] max_count {first['max_count']} -> {st['max_count']}, frames {st['frames_used']}/{st['frames_pool']}, continuity {res:.2e}")
+    assert res <= PP.TOL_CONT
+    pic.destroy()
+
+
 def test_species_table_and_anisotropic_cells():
     """Positive charge / heavier species and dx != dy != dz go through the same kernels."""
     wl = W.CONFIGS["khi"].scaled((16, 24, 8), cell=(1.0, 0.8, 1.25), dt=0.4)
