@@ -187,6 +187,32 @@ def test_append_loads_and_empty_supercells():
     pic.destroy()
 
 
+def test_load_more_particles_between_steps():
+    """pic_load_particles after stepping appends to the cell-sorted state (ids continue)."""
+    wl = W.CONFIGS["khi"].scaled((16, 16, 16))
+    parts, fields = W.make_particles(wl), W.make_fields(wl)
+    keys = ("x", "y", "z", "ux", "uy", "uz", "w", "species")
+    perm = torch.randperm(parts.n, generator=torch.Generator().manual_seed(3))
+    half = [W.ParticleChunk(*(getattr(parts, k)[idx] for k in keys)) for idx in (perm[: parts.n // 2], perm[parts.n // 2:])]
+    from paper_2110_08650_b200.binding import Pic
+    import oracle
+    pic = Pic(wl.grid, wl.cell, wl.dt, wl.supercell, wl.shape_order, max_particles=parts.n)
+    orc = oracle.Oracle(wl.grid, wl.cell, wl.dt, wl.supercell, wl.shape_order)
+    pic.set_fields(fields.cuda())
+    orc.set_fields(fields.numpy())
+    for h in half:
+        g = h.to("cuda:0")
+        pic.load_particles(*(getattr(g, k) for k in keys))
+        orc.load_particles(*(getattr(h, k).numpy() for k in keys[:7]), species=h.species.numpy())
+        pic.step(2)
+        assert orc.step(2) == 0
+    rep = PP.compare(wl, orc, pic, 4, 0.01)
+    print(f"\n[load between steps] {rep}")
+    assert rep.max_dx <= 4 * PP.TOL_X and rep.max_du_rel <= 4 * PP.TOL_U and rep.j_err_rel <= 4 * PP.TOL_J1
+    assert rep.n_member_mismatch == 0
+    pic.destroy()
+
+
 def test_roundtrip_without_step():
     """load -> get returns the same multiset, exactly (positions are integer + fp32 fraction)."""
     wl = W.CONFIGS["thermal_128"].scaled((16, 16, 8), ppc=5)
