@@ -244,6 +244,7 @@ def run_ours(args):
         pic.set_option("tma", args.tma)
         pic.set_option("deposit", args.deposit)
         pic.set_option("segment", args.segment)
+        pic.set_option("two_phase", args.two_phase)
         return pic
 
     # ---------------------------------------------------------------- device-resident throughput
@@ -336,6 +337,7 @@ def main():
     ap.add_argument("--tma", type=int, default=1)
     ap.add_argument("--deposit", type=int, default=1, help="1 fixed-point integer atomics, 0 float CAS atomics")
     ap.add_argument("--segment", type=int, default=3, help="work-item length in quarters of the mean cell population")
+    ap.add_argument("--two-phase", type=int, default=1, help="1: per-cell stencil in registers (two-phase items), 0: gather per particle from the shared tile")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -399,6 +399,8 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     d.pid[0] = (uint32_t*)(w + L.pid0); d.pid[1] = (uint32_t*)(w + L.pid1);
     d.cur = 0;
     d.seg_num = 3;
+    d.two_phase = 1;
+    d.order = shape_order;
     d.n_frames = L.n_frames;
     d.free_stack = (int*)(w + L.free_stack);
     d.tbl_pool = (int*)(w + L.tbl_pool); d.tbl_pool_size = L.tbl_pool_size;
@@ -614,6 +616,7 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
     if (!c || !key) return PIC_EINVAL;
     if (!strcmp(key, "tma")) { c->use_tma = value != 0; return PIC_OK; }
     if (!strcmp(key, "graph")) { c->use_graph = value != 0; return PIC_OK; }
+    if (!strcmp(key, "two_phase")) { c->d.two_phase = value != 0; return PIC_OK; }   // before loading particles
     if (!strcmp(key, "segment")) {
         if (value < 2 || value > 16) return fail(c, PIC_EINVAL, "pic_set_option: segment must be in 2..16");
         c->d.seg_num = (int)value;      // takes effect at the next sort (load or step)

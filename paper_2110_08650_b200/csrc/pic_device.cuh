@@ -69,6 +69,30 @@ __device__ __forceinline__ void ffma2(float& d0, float& d1, float a0, float a1, 
     asm("mov.b64 {%0, %1}, %2;" : "=f"(d0), "=f"(d1) : "l"(rc));
 }
 
+typedef unsigned long long f32x2;      // two floats in one 64-bit register pair
+__device__ __forceinline__ f32x2 pack2(float lo, float hi)
+{
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
 // One staggered component: F(X) = sum F[i,j,k] Wx Wy Wz.
 // (Pairing rows with packed FMAs was measured: no gain, 2.93 vs 2.89 ms.)
 template <int O>
@@ -93,6 +117,16 @@ __device__ __forceinline__ float gather1(const float* __restrict__ t, const floa
     return acc;
 }
 
+// ---- per-cell stencil windows (two-phase gather) -----------------------------------------------
+// For every particle of one cell the nodes a component needs along one axis lie in a fixed window:
+// O+1 nodes where the first node does not depend on the particle (CIC unstaggered, TSC staggered, PQS
+// unstaggered), O+2 nodes where it can take two values (the other three cases; the unused node gets weight 0).
+template <int O, bool ST> struct AxisWin {
+    static constexpr bool JIT = (O & 1) ? ST : !ST;          // first node depends on the particle
+    static constexpr int W = JIT ? O + 2 : O + 1;            // nodes in the window
+    static constexpr int LOW = (O == 1) ? (ST ? -1 : 0) : (O == 2) ? -1 : (ST ? -2 : -1);   // first node, cell-relative
+};
+
 // Place the O+1 weights of a shape evaluation into the W = O+2 wide Esirkepov window
 // (off = 0 or 1 = position of w[0] inside the window).
 template <int O>
@@ -112,6 +146,168 @@ __device__ __forceinline__ int wrapi(int i, int n)
     if (i >= n) i -= n;
     return i;
 }
+
+// weights of the window AxisWin<O,ST> for in-cell fraction f
+template <int O, bool ST>
+__device__ __forceinline__ void axis_weights(float f, float (&w)[AxisWin<O, ST>::W])
+{
+    float w0[O + 1];
+    const int b = shape<O>(ST ? f - 0.5f : f, w0);
+    if (AxisWin<O, ST>::JIT) {
+        float s[O + 2];
+        to_window<O>(w0, b - AxisWin<O, ST>::LOW, s);
+#pragma unroll
+        for (int t = 0; t < AxisWin<O, ST>::W; ++t) w[t] = s[t];
+    } else {
+#pragma unroll
+        for (int t = 0; t < AxisWin<O, ST>::W; ++t) w[t] = w0[t < O + 1 ? t : O];
+    }
+}
+
+// both weight sets (unstaggered / staggered lattice) of the three axes for one particle, plain and as
+// duplicated pairs {w,w} for the packed FMAs (unused members cost nothing)
+template <int O> struct CellWeights {
+    float u[3][AxisWin<O, false>::W];
+    float s[3][AxisWin<O, true>::W];
+    f32x2 u2[3][AxisWin<O, false>::W];
+    f32x2 s2[3][AxisWin<O, true>::W];
+    __device__ __forceinline__ void set(float fx, float fy, float fz)
+    {
+        axis_weights<O, false>(fx, u[0]); axis_weights<O, true>(fx, s[0]);
+        axis_weights<O, false>(fy, u[1]); axis_weights<O, true>(fy, s[1]);
+        axis_weights<O, false>(fz, u[2]); axis_weights<O, true>(fz, s[2]);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+#pragma unroll
+            for (int t = 0; t < AxisWin<O, false>::W; ++t) u2[a][t] = pack2(u[a][t], u[a][t]);
+#pragma unroll
+            for (int t = 0; t < AxisWin<O, true>::W; ++t) s2[a][t] = pack2(s[a][t], s[a][t]);
+        }
+    }
+    template <bool ST> __device__ __forceinline__ float get(int axis, int t) const
+    {
+        if constexpr (ST) return s[axis][t];
+        else return u[axis][t];
+    }
+    template <bool ST> __device__ __forceinline__ f32x2 get2(int axis, int t) const
+    {
+        if constexpr (ST) return s2[axis][t];
+        else return u2[axis][t];
+    }
+};
+
+// The nodes of field component C (0..5 = Ex,Ey,Ez,Bx,By,Bz) that the particles of ONE cell can touch,
+// held in registers: E_a is staggered along a, B_a along the two other axes.
+// The window is stored as register PAIRS of two z planes (PAIR 0; PAIR 2: the odd last plane stays
+// scalar) or of two y rows (PAIR 1), so that the x contraction runs as packed fma.rn.f32x2 (SASS FFMA2).
+template <int O, int C> struct CellStencil {
+    static constexpr bool STX = (C < 3) ? (C == 0) : (C != 3);
+    static constexpr bool STY = (C < 3) ? (C == 1) : (C != 4);
+    static constexpr bool STZ = (C < 3) ? (C == 2) : (C != 5);
+    using WX = AxisWin<O, STX>;
+    using WY = AxisWin<O, STY>;
+    using WZ = AxisWin<O, STZ>;
+    static constexpr int NX = WX::W, NY = WY::W, NZ = WZ::W;
+    static constexpr int PAIR = (NZ % 2 == 0) ? 0 : (NY % 2 == 0) ? 1 : 2;
+    static constexpr int NZP = NZ / 2, NYP = NY / 2;
+    f32x2 Pz[NZP][NY][NX];      // PAIR 0, 2: planes (2k, 2k+1)
+    float Lz[NY][NX];           // PAIR 2: last plane
+    f32x2 Py[NZ][NYP][NX];      // PAIR 1: rows (2k, 2k+1)
+
+    __device__ __forceinline__ void load(const float* __restrict__ sF, int cx, int cy, int cz)
+    {
+        using G = Geo<O>;
+        const float* t = sF + C * G::FCOMP + (cx + WX::LOW + G::FL) + (cy + WY::LOW + G::FL) * G::FPX +
+                         (cz + WZ::LOW + G::FL) * G::FPX * G::FNY;
+        float R[NZ][NY][NX];
+#pragma unroll
+        for (int c = 0; c < NZ; ++c)
+#pragma unroll
+            for (int b = 0; b < NY; ++b)
+#pragma unroll
+                for (int a = 0; a < NX; ++a) R[c][b][a] = t[(c * G::FNY + b) * G::FPX + a];
+        if constexpr (PAIR == 1) {
+#pragma unroll
+            for (int c = 0; c < NZ; ++c)
+#pragma unroll
+                for (int b = 0; b < NYP; ++b)
+#pragma unroll
+                    for (int a = 0; a < NX; ++a) Py[c][b][a] = pack2(R[c][2 * b][a], R[c][2 * b + 1][a]);
+        } else {
+#pragma unroll
+            for (int c = 0; c < NZP; ++c)
+#pragma unroll
+                for (int b = 0; b < NY; ++b)
+#pragma unroll
+                    for (int a = 0; a < NX; ++a) Pz[c][b][a] = pack2(R[2 * c][b][a], R[2 * c + 1][b][a]);
+            if constexpr (PAIR == 2) {
+#pragma unroll
+                for (int b = 0; b < NY; ++b)
+#pragma unroll
+                    for (int a = 0; a < NX; ++a) Lz[b][a] = R[NZ - 1][b][a];
+            }
+        }
+    }
+
+    // F(X) = sum F[i,j,k] Wx Wy Wz over the window (weights outside the particle's own O+1 nodes are 0)
+    __device__ __forceinline__ float eval(const CellWeights<O>& w) const
+    {
+        float acc = 0.0f;
+        if constexpr (PAIR == 1) {
+#pragma unroll
+            for (int c = 0; c < NZ; ++c) {
+                float az = 0.0f;
+#pragma unroll
+                for (int b = 0; b < NYP; ++b) {
+                    f32x2 ay = mul2(w.template get2<STX>(0, 0), Py[c][b][0]);
+#pragma unroll
+                    for (int a = 1; a < NX; ++a) ay = fma2(w.template get2<STX>(0, a), Py[c][b][a], ay);
+                    float y0, y1;
+                    unpack2(ay, y0, y1);
+                    az = fmaf(w.template get<STY>(1, 2 * b), y0, az);
+                    az = fmaf(w.template get<STY>(1, 2 * b + 1), y1, az);
+                }
+                acc = fmaf(w.template get<STZ>(2, c), az, acc);
+            }
+        } else {
+#pragma unroll
+            for (int c = 0; c < NZP; ++c) {
+                f32x2 az = 0;
+#pragma unroll
+                for (int b = 0; b < NY; ++b) {
+                    f32x2 ay = mul2(w.template get2<STX>(0, 0), Pz[c][b][0]);
+#pragma unroll
+                    for (int a = 1; a < NX; ++a) ay = fma2(w.template get2<STX>(0, a), Pz[c][b][a], ay);
+                    az = (b == 0) ? mul2(w.template get2<STY>(1, 0), ay) : fma2(w.template get2<STY>(1, b), ay, az);
+                }
+                float z0, z1;
+                unpack2(az, z0, z1);
+                acc = fmaf(w.template get<STZ>(2, 2 * c), z0, acc);
+                acc = fmaf(w.template get<STZ>(2, 2 * c + 1), z1, acc);
+            }
+            if constexpr (PAIR == 2) {
+                float az = 0.0f;
+#pragma unroll
+                for (int b = 0; b < NY; ++b) {
+                    float ay = 0.0f;
+#pragma unroll
+                    for (int a = 0; a < NX; ++a) ay = fmaf(w.template get<STX>(0, a), Lz[b][a], ay);
+                    az = fmaf(w.template get<STY>(1, b), ay, az);
+                }
+                acc = fmaf(w.template get<STZ>(2, NZ - 1), az, acc);
+            }
+        }
+        return acc;
+    }
+};
+
+// 16-byte asynchronous copy global -> shared (LDGSTS), bypassing L1 and the register file
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(gmem)
+                 : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 // ------------------------------------------------------------------ TMA + mbarrier (PTX)
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }

@@ -53,6 +53,8 @@ struct PicDev {
     float4* rec[2];
     uint32_t* pid[2];
     int cur;                     // pool holding the current state
+    int two_phase;               // 1: gather per item with the cell's stencil in registers
+    int order;                   // shape order (host copy for kernels that are not templated on it)
     int seg_num;                 // work-item length target in quarters of the mean cell population (2..16)
     int n_frames;
     int* free_stack;             // [n_frames] frames returned by shrinking supercells
@@ -97,10 +99,19 @@ struct PicDev {
 
 // Work items of the step kernel: a cell of n particles is cut into ceil(n/T) segments, with T about
 // 3/4 of the supercell's mean cell population (measured optimum of balance vs. flushes).
-__host__ __device__ inline int pic_segment_target(int supercell_count, int seg_num)
+// Two-phase path: an item's positions and gathered fields sit in shared memory, so an item holds at
+// most PIC_ITEM_LMAX particles (what fits beside the tiles with two CTAs per SM) and is flushed once.
+#define PIC_ITEM_LMAX(O) ((O) == 3 ? 6 : 11)
+#define PIC_ITEMCAP 1024         // work items per supercell: <= 256 + count/T
+
+// Work-item length target; lmax > 0 caps it where the supercell's item list still fits PIC_ITEMCAP
+// (count <= 768*lmax); more crowded supercells keep longer items and take the one-phase path.
+__host__ __device__ inline int pic_segment_target(int supercell_count, int seg_num, int lmax)
 {
-    const int t = (seg_num * supercell_count + 1023) / 1024;     // seg_num/4 of the mean cell population
-    return t < 4 ? 4 : t;
+    int t = (seg_num * supercell_count + 1023) / 1024;     // seg_num/4 of the mean cell population
+    if (t < 4) t = 4;
+    if (lmax > 0 && supercell_count <= 768 * lmax && t > lmax) t = lmax;
+    return t;
 }
 
 __host__ __device__ inline uint32_t pic_pack_bits(int local_cell, int species)

@@ -16,11 +16,10 @@
 
 namespace {
 
-#define PIC_XSTAGE 256     // leavers staged in shared memory per CTA before one bulk append
-#define PIC_SLOWCAP 768    // queued out-of-window particles per CTA
+#define PIC_XSTAGE 128     // leavers staged in shared memory per CTA before one bulk append
+#define PIC_SLOWCAP_OF(O) ((O) == 3 ? 256 : 64)   // queued out-of-window particles per CTA (then: overflow queue)
 #define PIC_STEP_THREADS 128   // 2 CTAs of 4 warps per SM: ~250 registers per thread for the accumulators
 #define PIC_DIRECT_BELOW 1536   // supercells with fewer particles (< 6 per cell) take the per-particle path
-#define PIC_ITEMCAP 800    // work items (cell segments) per supercell: <= 256 + count/T, T >= count/512
 
 // Esirkepov density decomposition of one component, straight into the
 // shared tile, with a per-particle window [lo, lo+O+2):
@@ -81,8 +80,17 @@ template <int O, bool FIX> struct StepSmem {
     static constexpr int OFF_XID = OFF_XREC + PIC_XSTAGE * 32;   // u32[XSTAGE]
     static constexpr int OFF_XDST = OFF_XID + PIC_XSTAGE * 4;    // int[XSTAGE]
     static constexpr int OFF_SLOW = OFF_XDST + PIC_XSTAGE * 4;   // float[SLOWCAP][8]
-    static constexpr int OFF_ITEMS = OFF_SLOW + PIC_SLOWCAP * 32; // int2[ITEMCAP]
-    static constexpr int TOTAL = OFF_ITEMS + PIC_ITEMCAP * 8;
+    static constexpr int SLOWCAP = PIC_SLOWCAP_OF(O);
+    static constexpr int OFF_ITEMS = OFF_SLOW + SLOWCAP * 32;    // int2[ITEMCAP]
+    // two-phase path: per thread and item slot the record's first half {fx,fy,fz,w} and NSLOT floats
+    // (gathered components on their way to the Boris push, then the new position on its way to the deposit)
+    static constexpr int LMAX = PIC_ITEM_LMAX(O);
+    static constexpr int NSLOT = (O == 3) ? 5 : 3;
+    static constexpr int OFF_STGP = (OFF_ITEMS + PIC_ITEMCAP * 8 + 15) / 16 * 16;   // float4[LMAX][128]
+    static constexpr int OFF_STGF = OFF_STGP + LMAX * 16 * PIC_STEP_THREADS;         // float[LMAX][NSLOT][128]
+    static constexpr int TOTAL = OFF_STGF + LMAX * NSLOT * 4 * PIC_STEP_THREADS;
+    // two CTAs per SM: 228 KB of shared memory, 1 KB reserved per CTA, 64 B of static variables
+    static_assert(!FIX || 2 * (TOTAL + 1024 + 64) <= 228 * 1024, "two step CTAs must fit one SM");
 };
 
 // One out-of-window particle, straight into the tile (all 32 lanes of the warp take part; lanes
@@ -154,16 +162,12 @@ __device__ __forceinline__ void flush1(float* sJ, int* sJhi, int* sJlo, int off,
     else if (v != 0.0f) atomicAdd(sJ + off, v);
 }
 
-// a2 + a3 for one particle: gather E,B at x^n, Boris push (step 4), move
-// (step 5) and the split of the new position into cell shift + in-cell fraction (reading S19).
+// a2 for one particle: gather E,B at x^n from the shared tile.
 template <int O>
-__device__ __forceinline__ void push_particle(const PicDev& d, const float* sF, int cx, int cy, int cz, int sp,
-                                              const float4& P, const float4& M, float (&un)[3], float (&fn)[3],
-                                              float (&x1)[3], int (&sh)[3])
+__device__ __forceinline__ void gather_particle(const float* sF, int cx, int cy, int cz, const float4& P,
+                                                float (&E)[3], float (&B)[3])
 {
     using G = Geo<O>;
-    // ---- a2: gather at x^n
-    float E[3], B[3];
     {
         float wu[3][O + 1], ws[3][O + 1];
         int bu[3], bs[3];
@@ -183,8 +187,14 @@ __device__ __forceinline__ void push_particle(const PicDev& d, const float* sF, 
         B[1] = gather1<O>(sF + 4 * G::FCOMP + sx_ + uy_ + sz_, ws[0], wu[1], ws[2]);
         B[2] = gather1<O>(sF + 5 * G::FCOMP + sx_ + sy_ + uz_, ws[0], ws[1], wu[2]);
     }
+}
 
-    // ---- a3: Boris push and move (step 5)
+// a3 for one particle: Boris push, move (step 5) and the split of the new
+// position into cell shift + in-cell fraction (reading S19).
+__device__ __forceinline__ void boris_move(const PicDev& d, int sp, const float4& P, const float4& M,
+                                           const float (&E)[3], const float (&B)[3], float (&un)[3], float (&fn)[3],
+                                           float (&x1)[3], int (&sh)[3])
+{
     const float h = d.h[sp];
     const float umx = fmaf(h, E[0], M.x), umy = fmaf(h, E[1], M.y), umz = fmaf(h, E[2], M.z);
     const float igm = rsqrtf(1.0f + umx * umx + umy * umy + umz * umz);
@@ -220,6 +230,17 @@ __device__ __forceinline__ void push_particle(const PicDev& d, const float* sF, 
     }
     if (far) atomicOr(d.ctr + CTR_ERROR, PIC_DEV_MOVED_TOO_FAR);
     un[0] = unx; un[1] = uny; un[2] = unz;
+}
+
+// a2 + a3 for one particle, gathering from the shared E/B tile.
+template <int O>
+__device__ __forceinline__ void push_particle(const PicDev& d, const float* sF, int cx, int cy, int cz, int sp,
+                                              const float4& P, const float4& M, float (&un)[3], float (&fn)[3],
+                                              float (&x1)[3], int (&sh)[3])
+{
+    float E[3], B[3];
+    gather_particle<O>(sF, cx, cy, cz, P, E, B);
+    boris_move(d, sp, P, M, E, B, un, fn, x1, sh);
 }
 
 // a5 for one particle: new local cell and destination supercell; stayers are written back in place
@@ -266,18 +287,77 @@ __device__ __forceinline__ void finish_particle(const PicDev& d, float4* rec, si
     }
 }
 
+// ------------------------------------------------------------------ two-phase gather
+// The stencils of the components in MASK for one cell (members outside MASK are never touched and cost nothing).
+template <int O, int MASK> struct StencilSet {
+    CellStencil<O, 0> c0; CellStencil<O, 1> c1; CellStencil<O, 2> c2;
+    CellStencil<O, 3> c3; CellStencil<O, 4> c4; CellStencil<O, 5> c5;
+    __device__ __forceinline__ void load(const float* sF, int cx, int cy, int cz)
+    {
+        if constexpr ((MASK & 1) != 0) c0.load(sF, cx, cy, cz);
+        if constexpr ((MASK & 2) != 0) c1.load(sF, cx, cy, cz);
+        if constexpr ((MASK & 4) != 0) c2.load(sF, cx, cy, cz);
+        if constexpr ((MASK & 8) != 0) c3.load(sF, cx, cy, cz);
+        if constexpr ((MASK & 16) != 0) c4.load(sF, cx, cy, cz);
+        if constexpr ((MASK & 32) != 0) c5.load(sF, cx, cy, cz);
+    }
+    template <int C> __device__ __forceinline__ float eval(const CellWeights<O>& w) const
+    {
+        if constexpr (C == 0) return c0.eval(w);
+        else if constexpr (C == 1) return c1.eval(w);
+        else if constexpr (C == 2) return c2.eval(w);
+        else if constexpr (C == 3) return c3.eval(w);
+        else if constexpr (C == 4) return c4.eval(w);
+        else return c5.eval(w);
+    }
+};
+
+// One gather pass over the n particles of the thread's item: the components in MASK, each into its
+// staging slot (slot = component index).  stgP/stgF point at the thread's own column.
+template <int O, int MASK, int NSLOT>
+__device__ __forceinline__ void gather_pass(const float* sF, int cx, int cy, int cz, int n, const float4* stgP, float* stgF)
+{
+    constexpr int NT = PIC_STEP_THREADS;
+    StencilSet<O, MASK> st;
+    st.load(sF, cx, cy, cz);
+    for (int i = 0; i < n; ++i) {
+        const float4 P = stgP[i * NT];
+        CellWeights<O> w;
+        w.set(P.x, P.y, P.z);
+        float* o = stgF + i * NSLOT * NT;
+        if constexpr ((MASK & 1) != 0) o[0 * NT] = st.template eval<0>(w);
+        if constexpr ((MASK & 2) != 0) o[1 * NT] = st.template eval<1>(w);
+        if constexpr ((MASK & 4) != 0) o[2 * NT] = st.template eval<2>(w);
+        if constexpr ((MASK & 8) != 0) o[3 * NT] = st.template eval<3>(w);
+        if constexpr ((MASK & 16) != 0) o[4 * NT] = st.template eval<4>(w);
+        if constexpr ((MASK & 32) != 0) o[5 * NT] = st.template eval<5>(w);
+    }
+}
+
 // ------------------------------------------------------------------ the step kernel
-// SPARSE = false: supercells with >= PIC_DIRECT_BELOW particles, 128 threads, register sums per cell segment.
-// SPARSE = true : the others, 256 threads, one thread per particle straight into the tile.
-// Both variants are launched over all supercells; a CTA whose supercell belongs to the other one exits.
-template <int O, bool TMA, bool FIX, bool SPARSE>
-__global__ void __launch_bounds__(SPARSE ? 256 : PIC_STEP_THREADS, SPARSE ? 3 : 2)
+// MODE 2: supercells with >= PIC_DIRECT_BELOW particles whose work items fit the two-phase path (<= LMAX
+//         particles each): 128 threads, per-cell stencils and Esirkepov sums in registers.
+// MODE 0: more crowded supercells (or two_phase off): 128 threads, gather per particle from the shared
+//         tile, register sums per cell segment.
+// MODE 1: sparse supercells, 256 threads, one thread per particle straight into the tile.
+// Every variant is launched over all supercells; a CTA whose supercell belongs to another one exits.
+#define PIC_MODE_ONE 0
+#define PIC_MODE_SPARSE 1
+#define PIC_MODE_TWO 2
+template <int O, bool TMA, bool FIX, int MODE>
+__global__ void __launch_bounds__(MODE == PIC_MODE_SPARSE ? 256 : PIC_STEP_THREADS, MODE == PIC_MODE_SPARSE ? 3 : 2)
 pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
 {
+    constexpr bool SPARSE = MODE == PIC_MODE_SPARSE;
+    constexpr bool two_phase = MODE == PIC_MODE_TWO;
     constexpr int NT = SPARSE ? 256 : PIC_STEP_THREADS;
     {
         const int n = d.sc_count[blockIdx.x];
         if (n == 0 || (n < PIC_DIRECT_BELOW) != SPARSE) return;
+        if (!SPARSE) {
+            const bool fits_two = d.two_phase && pic_segment_target(n, d.seg_num, PIC_ITEM_LMAX(O)) <= PIC_ITEM_LMAX(O);
+            if (fits_two != two_phase) return;
+        }
     }
     using G = Geo<O>;
     using S = StepSmem<O, FIX>;
@@ -293,6 +373,8 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
     int* s_xdst = reinterpret_cast<int*>(smem_raw + S::OFF_XDST);
     float* s_slow = reinterpret_cast<float*>(smem_raw + S::OFF_SLOW);
     int2* s_items = reinterpret_cast<int2*>(smem_raw + S::OFF_ITEMS);
+    float4* s_stgP = reinterpret_cast<float4*>(smem_raw + S::OFF_STGP);
+    float* s_stgF = reinterpret_cast<float*>(smem_raw + S::OFF_STGF);
     __shared__ int s_xn, s_slown, s_xbase, s_next, s_nitems;
     __shared__ __align__(8) uint64_t s_bar;
 
@@ -339,7 +421,7 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
     // work items: every cell is cut into k = ceil(n/T) near-equal segments, T ~ 3/4 of the mean cell
     // population; cells come in the order the sort kernel fixed (by decreasing segment length), so
     // the 32 items a warp takes at a time hold similar numbers of particles
-    const int seg_T = pic_segment_target(s_off[256], d.seg_num);
+    const int seg_T = pic_segment_target(s_off[256], d.seg_num, d.two_phase ? PIC_ITEM_LMAX(O) : 0);
     if (!SPARSE)
     for (int t = tid; t < 256; t += NT) {
         const int c = d.cell_perm[(size_t)s * 256 + t];
@@ -421,13 +503,123 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
     }
     const int cx = lc & 7, cy = (lc >> 3) & 7, cz = lc >> 6;
     float Ax[3][4][4], Ay[3][4][4], Az[3][4][4];
-#pragma unroll
-    for (int i = 0; i < 3; ++i)
-#pragma unroll
-        for (int b = 0; b < 4; ++b)
-#pragma unroll
-            for (int c = 0; c < 4; ++c) Ax[i][b][c] = Ay[i][b][c] = Az[i][b][c] = 0.0f;
 
+    // a4 for one particle of the item: Esirkepov, accumulated in registers over the cell's window
+    // (nodes -1..2); a particle whose new position leaves the window is queued
+    auto deposit_in_window = [&](const float (&f0)[3], const float (&x1)[3], float qw) {
+        float S0[3][4], DS[3][4];
+        bool fits = true;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            float w0[O + 1], w1[O + 1], s1[4];
+            const int b0 = shape<O>(f0[a], w0);
+            const int b1 = shape<O>(x1[a], w1);
+            fits &= (b1 >= -1) & (b1 <= 2 - O);
+            place4<O>(w0, b0 + 1, S0[a]);
+            place4<O>(w1, b1 + 1, s1);
+#pragma unroll
+            for (int t = 0; t < 4; ++t) DS[a][t] = s1[t] - S0[a][t];
+        }
+        if (fits) {
+            accumulate1(Ax, -qw * jfs[0], DS[0], S0[1], DS[1], S0[2], DS[2]);
+            accumulate1(Ay, -qw * jfs[1], DS[1], S0[2], DS[2], S0[0], DS[0]);
+            accumulate1(Az, -qw * jfs[2], DS[2], S0[0], DS[0], S0[1], DS[1]);
+        } else {
+            const int k = atomicAdd(&s_slown, 1);
+            if (k < S::SLOWCAP) {
+                float* q = s_slow + 8 * k;
+                q[0] = f0[0]; q[1] = f0[1]; q[2] = f0[2];
+                q[3] = x1[0]; q[4] = x1[1]; q[5] = x1[2];
+                q[6] = qw; q[7] = __int_as_float(lc);
+            } else {            // queue full: hand the particle to pic_overflow_kernel
+                const int k2 = atomicAdd(d.ctr + CTR_OVF, 1);
+                if (k2 < d.ovf_cap) {
+                    d.ovf[2 * (size_t)k2] = make_float4(f0[0], f0[1], f0[2], qw);
+                    d.ovf[2 * (size_t)k2 + 1] = make_float4(x1[0], x1[1], x1[2], __int_as_float(lc | (s << 8)));
+                } else {
+                    atomicOr(d.ctr + CTR_ERROR, PIC_DEV_OVERFLOW_QUEUE_FULL);
+                }
+            }
+        }
+    };
+    auto zero_sums = [&]() {
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+#pragma unroll
+            for (int b = 0; b < 4; ++b)
+#pragma unroll
+                for (int c = 0; c < 4; ++c) Ax[i][b][c] = Ay[i][b][c] = Az[i][b][c] = 0.0f;
+    };
+
+    if constexpr (two_phase) {
+        // ---- two-phase item (<= LMAX particles).  Phase 1, a2 + a3 + a5: the cell's stencil of a few
+        // components at a time sits in REGISTERS while the thread walks its particles; gathered values
+        // wait in the thread's own shared-memory column.  Phase 2, a4: the register sums.  The two
+        // phases never hold their registers (stencils / sums) at the same time.
+        constexpr int LAST = (O == 1) ? 0x3f : (O == 2) ? 0x38 : 0x20;    // components gathered in the last pass
+        const int n = p_end - p;
+        float4* stgP = s_stgP + tid;
+        float* stgF = s_stgF + tid;
+        for (int i = 0; i < n; ++i) {
+            const size_t idx = (size_t)tbl[(p + i) >> 8] * PIC_FRAME + ((p + i) & (PIC_FRAME - 1));
+            cp_async16(stgP + i * NT, rec + 2 * idx);
+        }
+        cp_async_wait_all();
+        if constexpr (O == 2) gather_pass<O, 0x07, S::NSLOT>(sF, cx, cy, cz, n, stgP, stgF);
+        if constexpr (O == 3) {
+            gather_pass<O, 0x01, S::NSLOT>(sF, cx, cy, cz, n, stgP, stgF);
+            gather_pass<O, 0x02, S::NSLOT>(sF, cx, cy, cz, n, stgP, stgF);
+            gather_pass<O, 0x04, S::NSLOT>(sF, cx, cy, cz, n, stgP, stgF);
+            gather_pass<O, 0x08, S::NSLOT>(sF, cx, cy, cz, n, stgP, stgF);
+            gather_pass<O, 0x10, S::NSLOT>(sF, cx, cy, cz, n, stgP, stgF);
+        }
+        {
+            StencilSet<O, LAST> st;
+            st.load(sF, cx, cy, cz);
+            size_t idx_n = 0;
+            float4 Mn = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (n > 0) {
+                idx_n = (size_t)tbl[p >> 8] * PIC_FRAME + (p & (PIC_FRAME - 1));
+                Mn = rec[2 * idx_n + 1];
+            }
+            for (int i = 0; i < n; ++i) {
+                const size_t idx = idx_n;
+                const float4 M = Mn;
+                if (i + 1 < n) {
+                    idx_n = (size_t)tbl[(p + i + 1) >> 8] * PIC_FRAME + ((p + i + 1) & (PIC_FRAME - 1));
+                    Mn = rec[2 * idx_n + 1];
+                }
+                const float4 P = stgP[i * NT];
+                float* o = stgF + i * S::NSLOT * NT;
+                CellWeights<O> w;
+                w.set(P.x, P.y, P.z);
+                float E[3], B[3];
+                if constexpr ((LAST & 1) != 0) E[0] = st.template eval<0>(w); else E[0] = o[0 * NT];
+                if constexpr ((LAST & 2) != 0) E[1] = st.template eval<1>(w); else E[1] = o[1 * NT];
+                if constexpr ((LAST & 4) != 0) E[2] = st.template eval<2>(w); else E[2] = o[2 * NT];
+                if constexpr ((LAST & 8) != 0) B[0] = st.template eval<3>(w); else B[0] = o[3 * NT];
+                if constexpr ((LAST & 16) != 0) B[1] = st.template eval<4>(w); else B[1] = o[4 * NT];
+                B[2] = st.template eval<5>(w);
+                const int sp = (__float_as_uint(M.w) >> 16) & 0xff;
+                float un[3], fn[3], x1[3];
+                int sh[3];
+                boris_move(d, sp, P, M, E, B, un, fn, x1, sh);
+                o[0 * NT] = x1[0]; o[1 * NT] = x1[1]; o[2 * NT] = x1[2];
+                reinterpret_cast<float*>(stgP + i * NT)[3] = d.q[sp] * P.w;
+                finish_particle(d, rec, idx, s, ssx, ssy, ssz, cx, cy, cz, sp, P, M, un, fn, sh, s_hist, &s_xn, s_xrec,
+                                s_xid, s_xdst);
+            }
+        }
+        zero_sums();
+        for (int i = 0; i < n; ++i) {
+            const float4 P = stgP[i * NT];     // {f0, q*w}
+            const float* o = stgF + i * S::NSLOT * NT;
+            const float f0[3] = {P.x, P.y, P.z};
+            const float x1[3] = {o[0 * NT], o[1 * NT], o[2 * NT]};
+            deposit_in_window(f0, x1, P.w);
+        }
+    } else {
+    zero_sums();
     // the next record is fetched while the current particle is processed
     size_t idx_n = 0;
     float4 Pn = make_float4(0.f, 0.f, 0.f, 0.f), Mn = Pn;
@@ -445,58 +637,59 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
             Mn = rec[2 * idx_n + 1];
         }
         const int sp = (__float_as_uint(M.w) >> 16) & 0xff;
-
         float un[3], fn[3], x1[3];
         int sh[3];
         push_particle<O>(d, sF, cx, cy, cz, sp, P, M, un, fn, x1, sh);
         const float f0[3] = {P.x, P.y, P.z};
-
-
-        // ---- a4: Esirkepov, accumulated in registers over the cell's window (nodes -1..2)
-        {
-            float S0[3][4], DS[3][4];
-            bool fits = true;
-#pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                float w0[O + 1], w1[O + 1], s1[4];
-                const int b0 = shape<O>(f0[a], w0);
-                const int b1 = shape<O>(x1[a], w1);
-                fits &= (b1 >= -1) & (b1 <= 2 - O);
-                place4<O>(w0, b0 + 1, S0[a]);
-                place4<O>(w1, b1 + 1, s1);
-#pragma unroll
-                for (int t = 0; t < 4; ++t) DS[a][t] = s1[t] - S0[a][t];
-            }
-            const float qw = d.q[sp] * P.w;
-            if (fits) {
-                accumulate1(Ax, -qw * jfs[0], DS[0], S0[1], DS[1], S0[2], DS[2]);
-                accumulate1(Ay, -qw * jfs[1], DS[1], S0[2], DS[2], S0[0], DS[0]);
-                accumulate1(Az, -qw * jfs[2], DS[2], S0[0], DS[0], S0[1], DS[1]);
-            } else {
-                const int k = atomicAdd(&s_slown, 1);
-                if (k < PIC_SLOWCAP) {
-                    float* q = s_slow + 8 * k;
-                    q[0] = f0[0]; q[1] = f0[1]; q[2] = f0[2];
-                    q[3] = x1[0]; q[4] = x1[1]; q[5] = x1[2];
-                    q[6] = qw; q[7] = __int_as_float(lc);
-                } else {            // queue full: hand the particle to pic_overflow_kernel
-                    const int k2 = atomicAdd(d.ctr + CTR_OVF, 1);
-                    if (k2 < d.ovf_cap) {
-                        d.ovf[2 * (size_t)k2] = make_float4(f0[0], f0[1], f0[2], qw);
-                        d.ovf[2 * (size_t)k2 + 1] = make_float4(x1[0], x1[1], x1[2], __int_as_float(lc | (s << 8)));
-                    } else {
-                        atomicOr(d.ctr + CTR_ERROR, PIC_DEV_OVERFLOW_QUEUE_FULL);
-                    }
-                }
-            }
-        }
-
+        deposit_in_window(f0, x1, d.q[sp] * P.w);
         finish_particle(d, rec, idx, s, ssx, ssy, ssz, cx, cy, cz, sp, P, M, un, fn, sh, s_hist, &s_xn, s_xrec, s_xid, s_xdst);
     }
+    }
 
-    // ---- a4: one flush of the segment's 3 x 48 partial sums into the shared tile (warp-synchronous)
+    // ---- a4: one flush of the item's 3 x 48 partial sums into the shared tile
     if (ibase + lane < n_items) {
         const int j0 = (cx - 1 + G::JL) * SX + (cy - 1 + G::JL) * SY + (cz - 1 + G::JL) * SZ;
+        if constexpr (two_phase) {
+            // through the thread's own staging column and a rolled loop: the unrolled form is 18 KB of
+            // code, which together with the three phase loops overflows the 32 KB instruction cache
+            // rows (i,b) of four values: the first LMAX rows in the float4 slots, the rest in the float slots
+            static_assert(S::LMAX + S::LMAX * S::NSLOT / 4 >= 12, "staging column too short for one component's sums");
+            float4* colP = s_stgP + tid;
+            float* colF = s_stgF + tid;
+#pragma unroll 1
+            for (int comp = 0; comp < 3; ++comp) {
+#pragma unroll
+                for (int r = 0; r < 12; ++r) {
+                    const int i = r >> 2, b = r & 3;
+                    float v[4];
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) v[c] = comp == 0 ? Ax[i][b][c] : comp == 1 ? Ay[i][b][c] : Az[i][b][c];
+                    if (r < S::LMAX) colP[r * NT] = make_float4(v[0], v[1], v[2], v[3]);
+                    else {
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) colF[((r - S::LMAX) * 4 + c) * NT] = v[c];
+                    }
+                }
+                const int sa = comp == 0 ? SX : comp == 1 ? SY : SZ;
+                const int sb = comp == 0 ? SY : comp == 1 ? SZ : SX;
+                const int sc = comp == 0 ? SZ : comp == 1 ? SX : SY;
+                const int cbase = j0 + comp * G::JCOMP;
+#pragma unroll
+                for (int r = 0; r < 12; ++r) {
+                    const int i = r >> 2, b = r & 3;
+                    float v[4];
+                    if (r < S::LMAX) {
+                        const float4 q = colP[r * NT];
+                        v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
+                    } else {
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) v[c] = colF[((r - S::LMAX) * 4 + c) * NT];
+                    }
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) flush1<FIX>(sJ, sJhi, sJlo, cbase + i * sa + b * sb + c * sc, v[c]);
+                }
+            }
+        } else {
 #pragma unroll
         for (int i = 0; i < 3; ++i)
 #pragma unroll
@@ -507,13 +700,14 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
                     flush1<FIX>(sJ, sJhi, sJlo, j0 + 1 * G::JCOMP + i * SY + b * SZ + c * SX, Ay[i][b][c]);
                     flush1<FIX>(sJ, sJhi, sJlo, j0 + 2 * G::JCOMP + i * SZ + b * SX + c * SY, Az[i][b][c]);
                 }
+        }
     }
     }   // next batch of work items
     __syncthreads();
 
     // ---- a4: queued out-of-window particles, one thread each
     {
-        const int n_slow = min(s_slown, PIC_SLOWCAP);
+        const int n_slow = min(s_slown, S::SLOWCAP);
         for (int base = 0; base < n_slow; base += NT) {
             if (base + (tid & ~31) < n_slow) {          // warp-uniform
                 const int e = base + tid;
@@ -757,7 +951,7 @@ __global__ void __launch_bounds__(PIC_FRAME) pic_sort_kernel(const PicDev d)
     // work items of the next step: cell c is cut into k = ceil(n/T) segments of ~n/k particles; order
     // the cells by decreasing segment length (ties by index) and publish the first item of each
     if (total >= PIC_DIRECT_BELOW) {   // block-uniform; the per-particle path needs no work items
-    const int seg_T = pic_segment_target(total, d.seg_num);
+    const int seg_T = pic_segment_target(total, d.seg_num, d.two_phase ? PIC_ITEM_LMAX(d.order) : 0);
     const int k = (cnt + seg_T - 1) / seg_T;
     const int seglen = k ? (cnt + k - 1) / k : 0;
     __syncthreads();               // s_cnt is complete; reuse it for the keys
@@ -852,26 +1046,33 @@ __global__ void __launch_bounds__(PIC_FRAME) pic_sort_kernel(const PicDev d)
 
 }  // namespace
 
-template <int O, bool TMA, bool FIX, bool SPARSE>
+template <int O, bool TMA, bool FIX, int MODE>
 static cudaError_t launch_step_one(const PicDev& d, const CUtensorMap& map, cudaStream_t st)
 {
     static bool configured = false;     // opt in to > 48 KB of dynamic shared memory once
-    constexpr int bytes = SPARSE ? StepSmem<O, FIX>::OFF_SLOW : StepSmem<O, FIX>::TOTAL;
+    constexpr bool SPARSE = MODE == PIC_MODE_SPARSE;
+    constexpr int bytes = SPARSE ? StepSmem<O, FIX>::OFF_SLOW
+                                 : MODE == PIC_MODE_ONE ? StepSmem<O, FIX>::OFF_STGP : StepSmem<O, FIX>::TOTAL;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(pic_step_kernel<O, TMA, FIX, SPARSE>,
+        cudaError_t e = cudaFuncSetAttribute(pic_step_kernel<O, TMA, FIX, MODE>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    pic_step_kernel<O, TMA, FIX, SPARSE><<<d.nsc, SPARSE ? 256 : PIC_STEP_THREADS, bytes, st>>>(d, map);
+    pic_step_kernel<O, TMA, FIX, MODE><<<d.nsc, SPARSE ? 256 : PIC_STEP_THREADS, bytes, st>>>(d, map);
     return cudaGetLastError();
 }
 
 template <int O, bool TMA, bool FIX>
 static cudaError_t launch_step_variant(const PicDev& d, const CUtensorMap& map, cudaStream_t st, int64_t* launches)
 {
-    cudaError_t e = launch_step_one<O, TMA, FIX, false>(d, map, st);
-    if (e == cudaSuccess) e = launch_step_one<O, TMA, FIX, true>(d, map, st);
+    cudaError_t e = cudaSuccess;
+    if (d.two_phase) {
+        e = launch_step_one<O, TMA, FIX, PIC_MODE_TWO>(d, map, st);
+        ++*launches;
+    }
+    if (e == cudaSuccess) e = launch_step_one<O, TMA, FIX, PIC_MODE_ONE>(d, map, st);
+    if (e == cudaSuccess) e = launch_step_one<O, TMA, FIX, PIC_MODE_SPARSE>(d, map, st);
     *launches += 2;
     return e;
 }
