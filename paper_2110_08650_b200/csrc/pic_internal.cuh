@@ -110,7 +110,7 @@ __host__ __device__ inline int pic_segment_target(int supercell_count, int seg_n
 {
     int t = (seg_num * supercell_count + 1023) / 1024;     // seg_num/4 of the mean cell population
     if (t < 4) t = 4;
-    if (lmax > 0 && supercell_count <= 768 * lmax && t > lmax) t = lmax;
+    if (lmax > 0 && supercell_count <= 768 * lmax) t = lmax;    // two-phase: items as long as the staging allows
     return t;
 }
 

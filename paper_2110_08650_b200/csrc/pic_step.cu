@@ -17,7 +17,7 @@
 namespace {
 
 #define PIC_XSTAGE 128     // leavers staged in shared memory per CTA before one bulk append
-#define PIC_SLOWCAP_OF(O) ((O) == 3 ? 256 : 64)   // queued out-of-window particles per CTA (then: overflow queue)
+#define PIC_SLOWCAP_OF(O) ((O) == 3 ? 256 : 32)   // queued out-of-window particles per CTA (then: overflow queue)
 #define PIC_STEP_THREADS 128   // 2 CTAs of 4 warps per SM: ~250 registers per thread for the accumulators
 #define PIC_DIRECT_BELOW 1536   // supercells with fewer particles (< 6 per cell) take the per-particle path
 
@@ -89,8 +89,9 @@ template <int O, bool FIX> struct StepSmem {
     static constexpr int OFF_STGP = (OFF_ITEMS + PIC_ITEMCAP * 8 + 15) / 16 * 16;   // float4[LMAX][128]
     static constexpr int OFF_STGF = OFF_STGP + LMAX * 16 * PIC_STEP_THREADS;         // float[LMAX][NSLOT][128]
     static constexpr int TOTAL = OFF_STGF + LMAX * NSLOT * 4 * PIC_STEP_THREADS;
-    // two CTAs per SM: 228 KB of shared memory, 1 KB reserved per CTA, 64 B of static variables
-    static_assert(!FIX || 2 * (TOTAL + 1024 + 64) <= 228 * 1024, "two step CTAs must fit one SM");
+    // two CTAs per SM: 228 KB of shared memory, 1 KB reserved per CTA, < 256 B of static variables
+    // (checked again at run time by launch_step_one: the kernel must reach 2 CTAs per SM)
+    static_assert(!FIX || 2 * (TOTAL + 1024 + 256) <= 228 * 1024, "two step CTAs must fit one SM");
 };
 
 // One out-of-window particle, straight into the tile (all 32 lanes of the warp take part; lanes
@@ -270,14 +271,13 @@ __device__ __forceinline__ void finish_particle(const PicDev& d, float4* rec, si
         const int dst = wrapi(ssx + dsx, d.nsx) + d.nsx * (wrapi(ssy + dsy, d.nsy) + d.nsy * wrapi(ssz + dsz, d.nsz));
         rec[2 * idx + 1] = make_float4(unx, uny, unz, __uint_as_float(nbits | PIC_LEFT_FLAG));   // hole
         M.w = __uint_as_float(nbits);
-        const uint32_t id = d.pid[d.cur][idx];
         const int k = atomicAdd(s_xn, 1);
-        if (k < PIC_XSTAGE) {
-            s_xrec[2 * k] = P; s_xrec[2 * k + 1] = M; s_xid[k] = id; s_xdst[k] = dst;
+        if (k < PIC_XSTAGE) {         // the id (a DRAM miss) is fetched by the bulk append, off the particle loop
+            s_xrec[2 * k] = P; s_xrec[2 * k + 1] = M; s_xid[k] = (uint32_t)idx; s_xdst[k] = dst;
         } else {                      // staging full: append directly
             const int xs = atomicAdd(d.ctr + CTR_EXCH, 1);
             if (xs < d.x_cap) {
-                d.x_rec[2 * (size_t)xs] = P; d.x_rec[2 * (size_t)xs + 1] = M; d.x_id[xs] = id; d.x_dst[xs] = dst;
+                d.x_rec[2 * (size_t)xs] = P; d.x_rec[2 * (size_t)xs + 1] = M; d.x_id[xs] = d.pid[d.cur][idx]; d.x_dst[xs] = dst;
             } else {
                 atomicOr(d.ctr + CTR_ERROR, PIC_DEV_EXCHANGE_OVERFLOW);
             }
@@ -314,14 +314,17 @@ template <int O, int MASK> struct StencilSet {
 
 // One gather pass over the n particles of the thread's item: the components in MASK, each into its
 // staging slot (slot = component index).  stgP/stgF point at the thread's own column.
-template <int O, int MASK, int NSLOT>
+template <int O, int MASK, int NSLOT, bool WAIT>
 __device__ __forceinline__ void gather_pass(const float* sF, int cx, int cy, int cz, int n, const float4* stgP, float* stgF)
 {
     constexpr int NT = PIC_STEP_THREADS;
     StencilSet<O, MASK> st;
     st.load(sF, cx, cy, cz);
+    if (WAIT) cp_async_wait_all();      // the item's records, requested before the stencil loads
+    float4 Pn = stgP[0];
     for (int i = 0; i < n; ++i) {
-        const float4 P = stgP[i * NT];
+        const float4 P = Pn;
+        Pn = stgP[(i + 1) * NT];        // next record's first half (slot LMAX is readable: start of the float slots)
         CellWeights<O> w;
         w.set(P.x, P.y, P.z);
         float* o = stgF + i * NSLOT * NT;
@@ -376,6 +379,7 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
     float4* s_stgP = reinterpret_cast<float4*>(smem_raw + S::OFF_STGP);
     float* s_stgF = reinterpret_cast<float*>(smem_raw + S::OFF_STGF);
     __shared__ int s_xn, s_slown, s_xbase, s_next, s_nitems;
+    __shared__ int s_tbl[two_phase ? (768 * PIC_ITEM_LMAX(O)) / PIC_FRAME + 3 : 1];
     __shared__ __align__(8) uint64_t s_bar;
 
     const int tid = threadIdx.x;
@@ -412,6 +416,10 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
     for (int e = tid; e < NJ; e += NT) sJhi[e] = 0;
     for (int t = tid; t < 257; t += NT) s_off[t] = d.cell_off[(size_t)s * 257 + t];
     for (int t = tid; t < 256; t += NT) s_hist[t] = 0;
+    if constexpr (two_phase) {
+        const int nfr = (d.sc_count[s] + PIC_FRAME - 1) / PIC_FRAME;
+        if (tid < nfr) s_tbl[tid] = d.tbl_pool[d.tbl_off[s] + tid];
+    }
     if (tid == 0) {
         s_xn = 0;
         s_slown = 0;
@@ -456,7 +464,9 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
     }
     const float jfs[3] = {d.jfx * fix_scale[0], d.jfy * fix_scale[1], d.jfz * fix_scale[2]};
 
+    // frame table: the two-phase variant (<= 768*LMAX particles, i.e. <= 35 frames) reads it from shared memory
     const int* tbl = d.tbl_pool + d.tbl_off[s];
+    if constexpr (two_phase) tbl = s_tbl;
     const int lane = tid & 31;
     const int n_items = s_nitems;
     constexpr int SX = 1, SY = G::JNX, SZ = G::JNX * G::JNY;
@@ -564,24 +574,25 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
             const size_t idx = (size_t)tbl[(p + i) >> 8] * PIC_FRAME + ((p + i) & (PIC_FRAME - 1));
             cp_async16(stgP + i * NT, rec + 2 * idx);
         }
-        cp_async_wait_all();
-        if constexpr (O == 2) gather_pass<O, 0x07, S::NSLOT>(sF, cx, cy, cz, n, stgP, stgF);
+        if constexpr (O == 2) gather_pass<O, 0x07, S::NSLOT, true>(sF, cx, cy, cz, n, stgP, stgF);
         if constexpr (O == 3) {
-            gather_pass<O, 0x01, S::NSLOT>(sF, cx, cy, cz, n, stgP, stgF);
-            gather_pass<O, 0x02, S::NSLOT>(sF, cx, cy, cz, n, stgP, stgF);
-            gather_pass<O, 0x04, S::NSLOT>(sF, cx, cy, cz, n, stgP, stgF);
-            gather_pass<O, 0x08, S::NSLOT>(sF, cx, cy, cz, n, stgP, stgF);
-            gather_pass<O, 0x10, S::NSLOT>(sF, cx, cy, cz, n, stgP, stgF);
+            gather_pass<O, 0x01, S::NSLOT, true>(sF, cx, cy, cz, n, stgP, stgF);
+            gather_pass<O, 0x02, S::NSLOT, false>(sF, cx, cy, cz, n, stgP, stgF);
+            gather_pass<O, 0x04, S::NSLOT, false>(sF, cx, cy, cz, n, stgP, stgF);
+            gather_pass<O, 0x08, S::NSLOT, false>(sF, cx, cy, cz, n, stgP, stgF);
+            gather_pass<O, 0x10, S::NSLOT, false>(sF, cx, cy, cz, n, stgP, stgF);
         }
         {
             StencilSet<O, LAST> st;
             st.load(sF, cx, cy, cz);
+            if constexpr (O == 1) cp_async_wait_all();
             size_t idx_n = 0;
             float4 Mn = make_float4(0.f, 0.f, 0.f, 0.f);
             if (n > 0) {
                 idx_n = (size_t)tbl[p >> 8] * PIC_FRAME + (p & (PIC_FRAME - 1));
                 Mn = rec[2 * idx_n + 1];
             }
+            float4 Pn = stgP[0];
             for (int i = 0; i < n; ++i) {
                 const size_t idx = idx_n;
                 const float4 M = Mn;
@@ -589,7 +600,8 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
                     idx_n = (size_t)tbl[(p + i + 1) >> 8] * PIC_FRAME + ((p + i + 1) & (PIC_FRAME - 1));
                     Mn = rec[2 * idx_n + 1];
                 }
-                const float4 P = stgP[i * NT];
+                const float4 P = Pn;
+                Pn = stgP[(i + 1) * NT];
                 float* o = stgF + i * S::NSLOT * NT;
                 CellWeights<O> w;
                 w.set(P.x, P.y, P.z);
@@ -611,11 +623,17 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
             }
         }
         zero_sums();
+        float4 Pn = stgP[0];     // {f0, q*w}
+        float xn[3] = {stgF[0 * NT], stgF[1 * NT], stgF[2 * NT]};
         for (int i = 0; i < n; ++i) {
-            const float4 P = stgP[i * NT];     // {f0, q*w}
-            const float* o = stgF + i * S::NSLOT * NT;
+            const float4 P = Pn;
             const float f0[3] = {P.x, P.y, P.z};
-            const float x1[3] = {o[0 * NT], o[1 * NT], o[2 * NT]};
+            const float x1[3] = {xn[0], xn[1], xn[2]};
+            Pn = stgP[(i + 1) * NT];
+            if (i + 1 < S::LMAX) {              // (keeps the prefetch inside the float slots)
+                const float* o = stgF + (i + 1) * S::NSLOT * NT;
+                xn[0] = o[0 * NT]; xn[1] = o[1 * NT]; xn[2] = o[2 * NT];
+            }
             deposit_in_window(f0, x1, P.w);
         }
     } else {
@@ -674,19 +692,24 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
                 const int sb = comp == 0 ? SY : comp == 1 ? SZ : SX;
                 const int sc = comp == 0 ? SZ : comp == 1 ? SX : SY;
                 const int cbase = j0 + comp * G::JCOMP;
+                constexpr int RP = S::LMAX < 12 ? S::LMAX : 12;     // rows kept in the float4 slots
+                float4 qn = colP[0];
+#pragma unroll 1
+                for (int r = 0; r < RP; ++r) {
+                    const float4 q = qn;
+                    qn = colP[(r + 1) * NT];
+                    const int rb = cbase + (r >> 2) * sa + (r & 3) * sb;
+                    flush1<FIX>(sJ, sJhi, sJlo, rb, q.x);
+                    flush1<FIX>(sJ, sJhi, sJlo, rb + sc, q.y);
+                    flush1<FIX>(sJ, sJhi, sJlo, rb + 2 * sc, q.z);
+                    flush1<FIX>(sJ, sJhi, sJlo, rb + 3 * sc, q.w);
+                }
+#pragma unroll 1
+                for (int r = RP; r < 12; ++r) {
+                    const float* f = colF + (r - RP) * 4 * NT;
+                    const int rb = cbase + (r >> 2) * sa + (r & 3) * sb;
 #pragma unroll
-                for (int r = 0; r < 12; ++r) {
-                    const int i = r >> 2, b = r & 3;
-                    float v[4];
-                    if (r < S::LMAX) {
-                        const float4 q = colP[r * NT];
-                        v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
-                    } else {
-#pragma unroll
-                        for (int c = 0; c < 4; ++c) v[c] = colF[((r - S::LMAX) * 4 + c) * NT];
-                    }
-#pragma unroll
-                    for (int c = 0; c < 4; ++c) flush1<FIX>(sJ, sJhi, sJlo, cbase + i * sa + b * sb + c * sc, v[c]);
+                    for (int c = 0; c < 4; ++c) flush1<FIX>(sJ, sJhi, sJlo, rb + c * sc, f[c * NT]);
                 }
             }
         } else {
@@ -733,7 +756,7 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
         if (xs < d.x_cap) {
             d.x_rec[2 * (size_t)xs] = s_xrec[2 * k];
             d.x_rec[2 * (size_t)xs + 1] = s_xrec[2 * k + 1];
-            d.x_id[xs] = s_xid[k];
+            d.x_id[xs] = d.pid[d.cur][s_xid[k]];      // staged: the record index (< 2^32 slots)
             d.x_dst[xs] = s_xdst[k];
         } else {
             atomicOr(d.ctr + CTR_ERROR, PIC_DEV_EXCHANGE_OVERFLOW);
@@ -1057,6 +1080,11 @@ static cudaError_t launch_step_one(const PicDev& d, const CUtensorMap& map, cuda
         cudaError_t e = cudaFuncSetAttribute(pic_step_kernel<O, TMA, FIX, MODE>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
         if (e != cudaSuccess) return e;
+        int ctas = 0;                   // the design point is two dense CTAs (three sparse ones) per SM
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas, pic_step_kernel<O, TMA, FIX, MODE>,
+                                                          SPARSE ? 256 : PIC_STEP_THREADS, bytes);
+        if (e != cudaSuccess) return e;
+        if (ctas < 2) return cudaErrorLaunchOutOfResources;
         configured = true;
     }
     pic_step_kernel<O, TMA, FIX, MODE><<<d.nsc, SPARSE ? 256 : PIC_STEP_THREADS, bytes, st>>>(d, map);
