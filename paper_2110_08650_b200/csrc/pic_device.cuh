@@ -372,4 +372,27 @@ __device__ __forceinline__ void fix_add(int* hi, int* lo, int off, float v)
     atomicAdd(lo + off, __float_as_int(t2) - PIC_FIX_MAGIC_BITS);
 }
 
+// two contributions at once: the float part of the split runs as packed f32x2 operations
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ void fix_add2(int* hi, int* lo, int off0, int off1, float v0, float v1)
+{
+    const f32x2 magic = pack2(PIC_FIX_MAGIC, PIC_FIX_MAGIC), nmagic = pack2(-PIC_FIX_MAGIC, -PIC_FIX_MAGIC);
+    const f32x2 v = pack2(v0, v1);
+    const f32x2 t = add2(v, magic);                                   // exact integers round(v)
+    const f32x2 nr = add2(add2(t, nmagic), pack2(-v0, -v1));          // -(v - round(v)), exact
+    const f32x2 t2 = fma2(nr, pack2(-(float)(1 << PIC_FIX_LO_BITS), -(float)(1 << PIC_FIX_LO_BITS)), magic);
+    float ta, tb, ua, ub;
+    unpack2(t, ta, tb);
+    unpack2(t2, ua, ub);
+    atomicAdd(hi + off0, __float_as_int(ta) - PIC_FIX_MAGIC_BITS);
+    atomicAdd(lo + off0, __float_as_int(ua) - PIC_FIX_MAGIC_BITS);
+    atomicAdd(hi + off1, __float_as_int(tb) - PIC_FIX_MAGIC_BITS);
+    atomicAdd(lo + off1, __float_as_int(ub) - PIC_FIX_MAGIC_BITS);
+}
+
 }  // namespace

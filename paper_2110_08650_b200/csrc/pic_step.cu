@@ -162,6 +162,15 @@ __device__ __forceinline__ void flush1(float* sJ, int* sJhi, int* sJlo, int off,
     if (FIX) fix_add(sJhi, sJlo, off, v);
     else if (v != 0.0f) atomicAdd(sJ + off, v);
 }
+template <bool FIX>
+__device__ __forceinline__ void flush2(float* sJ, int* sJhi, int* sJlo, int off0, int off1, float v0, float v1)
+{
+    if (FIX) fix_add2(sJhi, sJlo, off0, off1, v0, v1);
+    else {
+        if (v0 != 0.0f) atomicAdd(sJ + off0, v0);
+        if (v1 != 0.0f) atomicAdd(sJ + off1, v1);
+    }
+}
 
 // a2 for one particle: gather E,B at x^n from the shared tile.
 template <int O>
@@ -676,18 +685,20 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
             float* colF = s_stgF + tid;
 #pragma unroll 1
             for (int comp = 0; comp < 3; ++comp) {
+                auto stage_sums = [&](const float (&A)[3][4][4]) {
 #pragma unroll
-                for (int r = 0; r < 12; ++r) {
-                    const int i = r >> 2, b = r & 3;
-                    float v[4];
+                    for (int r = 0; r < 12; ++r) {
+                        const int i = r >> 2, b = r & 3;
+                        if (r < S::LMAX) colP[r * NT] = make_float4(A[i][b][0], A[i][b][1], A[i][b][2], A[i][b][3]);
+                        else {
 #pragma unroll
-                    for (int c = 0; c < 4; ++c) v[c] = comp == 0 ? Ax[i][b][c] : comp == 1 ? Ay[i][b][c] : Az[i][b][c];
-                    if (r < S::LMAX) colP[r * NT] = make_float4(v[0], v[1], v[2], v[3]);
-                    else {
-#pragma unroll
-                        for (int c = 0; c < 4; ++c) colF[((r - S::LMAX) * 4 + c) * NT] = v[c];
+                            for (int c = 0; c < 4; ++c) colF[((r - S::LMAX) * 4 + c) * NT] = A[i][b][c];
+                        }
                     }
-                }
+                };
+                if (comp == 0) stage_sums(Ax);
+                else if (comp == 1) stage_sums(Ay);
+                else stage_sums(Az);
                 const int sa = comp == 0 ? SX : comp == 1 ? SY : SZ;
                 const int sb = comp == 0 ? SY : comp == 1 ? SZ : SX;
                 const int sc = comp == 0 ? SZ : comp == 1 ? SX : SY;
@@ -699,17 +710,15 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
                     const float4 q = qn;
                     qn = colP[(r + 1) * NT];
                     const int rb = cbase + (r >> 2) * sa + (r & 3) * sb;
-                    flush1<FIX>(sJ, sJhi, sJlo, rb, q.x);
-                    flush1<FIX>(sJ, sJhi, sJlo, rb + sc, q.y);
-                    flush1<FIX>(sJ, sJhi, sJlo, rb + 2 * sc, q.z);
-                    flush1<FIX>(sJ, sJhi, sJlo, rb + 3 * sc, q.w);
+                    flush2<FIX>(sJ, sJhi, sJlo, rb, rb + sc, q.x, q.y);
+                    flush2<FIX>(sJ, sJhi, sJlo, rb + 2 * sc, rb + 3 * sc, q.z, q.w);
                 }
 #pragma unroll 1
                 for (int r = RP; r < 12; ++r) {
                     const float* f = colF + (r - RP) * 4 * NT;
                     const int rb = cbase + (r >> 2) * sa + (r & 3) * sb;
-#pragma unroll
-                    for (int c = 0; c < 4; ++c) flush1<FIX>(sJ, sJhi, sJlo, rb + c * sc, f[c * NT]);
+                    flush2<FIX>(sJ, sJhi, sJlo, rb, rb + sc, f[0], f[NT]);
+                    flush2<FIX>(sJ, sJhi, sJlo, rb + 2 * sc, rb + 3 * sc, f[2 * NT], f[3 * NT]);
                 }
             }
         } else {
