@@ -22,6 +22,10 @@ struct pic_ctx {
     cudaStream_t stream;
     bool have_fields;
     bool use_tma, use_graph, fixed_point;
+    bool fuse_sort;              // option "fuse_sort": the step kernel sorts its supercell first (default on)
+    bool dirty;                  // pool cur holds a stepped state whose sort is still pending
+    int* hist[2];                // the two cell histograms; d.cell_hist == hist[hist_cur]
+    int hist_cur;
     char* ws;
     uint64_t ws_bytes;
     std::string err;
@@ -42,7 +46,7 @@ namespace {
 
 struct Layout {
     uint64_t rec0, rec1, pid0, pid1, free_stack, tbl_pool, tbl_off, tbl_cap, sc_nframes, sc_count, sc_tail, sc_incoming,
-        cell_off, cell_hist, cell_perm, cell_kbase, x_rec, x_id, x_dst, ovf, ctr, ctr64, F, Fpad, J, J64, sc_offset, total;
+        sc_left, sc_next, cell_off, cell_hist, cell_perm, cell_kbase, x_rec, x_id, x_dst, ovf, ctr, ctr64, F, Fpad, J, J64, sc_offset, total;
     int n_frames, tbl_pool_size, x_cap, nsc;
 };
 
@@ -79,8 +83,10 @@ int compute_layout(const int32_t grid[3], const int32_t sc[3], int order, int64_
     L->sc_count = take(nsc * 4);
     L->sc_tail = take(nsc * 4);
     L->sc_incoming = take(nsc * 4);
+    L->sc_left = take(nsc * 4);
+    L->sc_next = take(nsc * 4);
     L->cell_off = take(nsc * 257 * 4);
-    L->cell_hist = take(nsc * 256 * 4);
+    L->cell_hist = take(2 * nsc * 256 * 4);      // two histograms (this step's, the previous step's)
     L->cell_perm = take(nsc * 256);
     L->cell_kbase = take(nsc * 256 * 2);
     L->x_rec = take(xcap * 32);
@@ -378,6 +384,8 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     c->have_fields = false;
     c->use_tma = true;
     c->use_graph = false;
+    c->fuse_sort = true;
+    c->dirty = false;
     c->fixed_point = true;
     c->tmap_ok = false;
     c->graph_exec = nullptr;
@@ -407,7 +415,12 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     d.tbl_off = (int*)(w + L.tbl_off); d.tbl_cap = (int*)(w + L.tbl_cap);
     d.sc_nframes = (int*)(w + L.sc_nframes); d.sc_count = (int*)(w + L.sc_count);
     d.sc_tail = (int*)(w + L.sc_tail); d.sc_incoming = (int*)(w + L.sc_incoming);
-    d.cell_off = (int*)(w + L.cell_off); d.cell_hist = (int*)(w + L.cell_hist);
+    d.sc_left = (int*)(w + L.sc_left); d.sc_next = (int*)(w + L.sc_next);
+    d.fused = 0;
+    d.cell_off = (int*)(w + L.cell_off);
+    c->hist[0] = (int*)(w + L.cell_hist); c->hist[1] = c->hist[0] + (size_t)L.nsc * 256;
+    c->hist_cur = 0;
+    d.cell_hist = c->hist[0]; d.cell_hist_prev = c->hist[1];
     d.cell_perm = (unsigned char*)(w + L.cell_perm);
     d.cell_kbase = (unsigned short*)(w + L.cell_kbase);
     d.x_rec = (float4*)(w + L.x_rec);
@@ -440,6 +453,8 @@ int32_t pic_set_species(pic_ctx* c, int32_t n, const double* q, const double* m)
     return PIC_OK;
 }
 
+static int ensure_sorted(pic_ctx* c);
+
 int32_t pic_load_particles(pic_ctx* c, int64_t n, const double* x, const double* y, const double* z,
                            const float* ux, const float* uy, const float* uz, const float* w,
                            const int32_t* species)
@@ -449,6 +464,10 @@ int32_t pic_load_particles(pic_ctx* c, int64_t n, const double* x, const double*
     if (n == 0) return PIC_OK;
     if (!x || !y || !z || !ux || !uy || !uz || !w) return fail(c, PIC_EINVAL, "pic_load_particles: NULL array");
     if (c->n_particles + n > c->max_particles) return fail(c, PIC_ENOMEM, "pic_load_particles: exceeds max_particles");
+    {
+        int rc = ensure_sorted(c);
+        if (rc != PIC_OK) return rc;
+    }
     LoadArgs a;
     a.x = x; a.y = y; a.z = z; a.ux = ux; a.uy = uy; a.uz = uz; a.w = w; a.species = species;
     a.n = n; a.id0 = (unsigned)c->n_particles;
@@ -492,11 +511,30 @@ int32_t pic_set_fields(pic_ctx* c, const float* Ex, const float* Ey, const float
     return PIC_OK;
 }
 
+// Sort the supercells of a stepped state (holes of leavers, appended arrivals) into the other pool.
+static int ensure_sorted(pic_ctx* c)
+{
+    if (!c->dirty) return PIC_OK;
+    c->d.fused = 0;
+    cudaError_t e = pic_launch_sort(c->d, c->stream, &c->launches);
+    if (e != cudaSuccess) return cuda_fail(c, e, "sort");
+    c->d.cur ^= 1;
+    c->dirty = false;
+    return PIC_OK;
+}
+
+// One step = [sort of the previous step's result, fused into the step kernel's prologue] + gather, push,
+// deposit, in-place write-back + convert J + make room + scatter leavers.  The state is left unsorted
+// ("dirty"); whoever needs the sorted arrangement (the next step, a load, a read-back) sorts it.
 static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
 {
     PicDev& d = c->d;
     const size_t ncell = (size_t)d.nx * d.ny * d.nz;
     for (int i = 0; i < n; ++i) {
+        if (c->dirty && !c->fuse_sort) {
+            int rc = ensure_sorted(c);
+            if (rc != PIC_OK) return rc;
+        }
         cudaError_t e = c->fixed_point ? cudaMemsetAsync(d.J64, 0, 3 * ncell * sizeof(long long), st)   // S16
                                        : cudaMemsetAsync(d.J, 0, 3 * ncell * sizeof(float), st);
         if (e == cudaSuccess) e = cudaMemsetAsync(d.ctr + CTR_EXCH, 0, sizeof(int), st);
@@ -507,7 +545,13 @@ static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
             if (e == cudaSuccess) e = cudaEventCreate(&ev1);
             if (e == cudaSuccess) e = cudaEventRecord(ev0, st);
         }
+        d.fused = c->dirty ? 1 : 0;
+        if (c->dirty) d.cur ^= 1;       // the kernel sorts pool cur^1 into pool cur and steps it there
+        d.cell_hist_prev = c->hist[c->hist_cur];        // pending histogram (all zero when the state is sorted)
+        c->hist_cur ^= 1;
+        d.cell_hist = c->hist[c->hist_cur];             // this step's
         if (e == cudaSuccess) e = pic_launch_step(d, c->order, c->use_tma && c->tmap_ok, c->fixed_point, c->tmap, st, &c->launches);
+        d.fused = 0;
         if (e == cudaSuccess && c->timing) {
             e = cudaEventRecord(ev1, st);
             c->events.push_back(ev0);
@@ -517,9 +561,8 @@ static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
         if (e == cudaSuccess && c->fixed_point) e = pic_launch_convert(d, st, &c->launches);
         if (e == cudaSuccess) e = pic_launch_prepare(d, st, &c->launches);
         if (e == cudaSuccess) e = pic_launch_scatter(d, st, &c->launches);
-        if (e == cudaSuccess) e = pic_launch_sort(d, st, &c->launches);
         if (e != cudaSuccess) return cuda_fail(c, e, "pic_step: launch");
-        d.cur ^= 1;     // the sorted state now lives in the other pool
+        c->dirty = true;
     }
     return PIC_OK;
 }
@@ -555,6 +598,10 @@ int32_t pic_get_particles(pic_ctx* c, int64_t capacity, int64_t* n_out, double* 
 {
     if (!c) return PIC_EINVAL;
     if (capacity < 0) return fail(c, PIC_EINVAL, "pic_get_particles: capacity < 0");
+    {
+        int rc = ensure_sorted(c);
+        if (rc != PIC_OK) return rc;
+    }
     const PicDev& d = c->d;
     pic_scan_counts_kernel<<<1, 1024, 0, c->stream>>>(d);
     GetArgs a;
@@ -577,6 +624,10 @@ int32_t pic_get_counts(pic_ctx* c, int32_t* per_supercell_count)
 {
     if (!c) return PIC_EINVAL;
     if (!per_supercell_count) return fail(c, PIC_EINVAL, "pic_get_counts: NULL");
+    {
+        int rc = ensure_sorted(c);
+        if (rc != PIC_OK) return rc;
+    }
     cudaError_t e = cudaMemcpyAsync(per_supercell_count, c->d.sc_count, (size_t)c->d.nsc * sizeof(int),
                                     cudaMemcpyDeviceToDevice, c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "pic_get_counts: cudaMemcpyAsync");
@@ -616,6 +667,7 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
     if (!c || !key) return PIC_EINVAL;
     if (!strcmp(key, "tma")) { c->use_tma = value != 0; return PIC_OK; }
     if (!strcmp(key, "graph")) { c->use_graph = value != 0; return PIC_OK; }
+    if (!strcmp(key, "fuse_sort")) { c->fuse_sort = value != 0; return PIC_OK; }
     if (!strcmp(key, "two_phase")) { c->d.two_phase = value != 0; return PIC_OK; }   // before loading particles
     if (!strcmp(key, "segment")) {
         if (value < 2 || value > 16) return fail(c, PIC_EINVAL, "pic_set_option: segment must be in 2..16");

@@ -66,10 +66,16 @@ struct PicDev {
     int* sc_count;               // [nsc] particles in the supercell
     int* sc_tail;                // [nsc] slots in use incl. holes of leavers and appended arrivals
     int* cell_off;               // [nsc][257] slot ranges of the local cells (sorted arrangement)
-    int* cell_hist;              // [nsc][256] particles per NEW local cell (stayers + arrivals), zero between steps
+    int* cell_hist;              // [nsc][256] particles per NEW local cell (stayers + arrivals), filled by this step
+    int* cell_hist_prev;         // the previous step's histogram, consumed (and cleared) by the fused sort: CTAs of one
+                                 // launch read it while others already add this step's leavers to cell_hist
     unsigned char* cell_perm;    // [nsc][256] local cells ordered by decreasing work-item length
     unsigned short* cell_kbase;  // [nsc][256] first work item of the cell at that position
     int* sc_incoming;            // [nsc] leavers headed here
+    int* sc_left;                // [nsc] leavers of the last step (written by the step kernel, consumed by prepare)
+    int* sc_next;                // [nsc] population after the pending sort (stayers + arrivals), set by prepare
+    int fused;                   // 1: pool cur^1 holds the stepped, not yet sorted state; the step kernel sorts its
+                                 //    supercell into pool cur first, 0: pool cur is sorted
     // exchange buffer for supercell leavers
     float4* x_rec;               // 2 float4 per entry
     uint32_t* x_id;

@@ -346,6 +346,170 @@ __device__ __forceinline__ void gather_pass(const float* sF, int cx, int cy, int
     }
 }
 
+// ------------------------------------------------------------------ sort fused into the step kernel's prologue
+// Exclusive scan over 256 counts held NT-strided in registers (entry tid*PER + k); two block barriers.
+template <int NT>
+__device__ __forceinline__ void block_excl_scan256(int (&v)[256 / NT], int& total, int* s_w, int tid)
+{
+    constexpr int PER = 256 / NT, NW = NT / 32;
+    const int lane = tid & 31, warp = tid >> 5;
+    int sum = 0;
+#pragma unroll
+    for (int k = 0; k < PER; ++k) sum += v[k];
+    int inc = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    __syncthreads();               // s_w may still be read from an earlier scan
+    if (lane == 31) s_w[warp] = inc;
+    __syncthreads();
+    int wb = 0;
+    total = 0;
+#pragma unroll
+    for (int w = 0; w < NW; ++w) {
+        const int x = s_w[w];
+        if (w < warp) wb += x;
+        total += x;
+    }
+    int off = wb + inc - sum;
+#pragma unroll
+    for (int k = 0; k < PER; ++k) {
+        const int c = v[k];
+        v[k] = off;
+        off += c;
+    }
+}
+
+// The counting sort of pic_sort_kernel for ONE supercell, run by the step CTA before it steps the
+// supercell: pool cur^1 (stayers, holes of leavers, appended arrivals) -> pool cur, sorted by cell.
+// Leaves the cell ranges in s_off[0..256] (shared), publishes the new count, clears the global histogram,
+// returns frames the supercell no longer needs.  s_cur: 256 ints of scratch; s_w: 16 ints of scratch.
+template <int NT>
+__device__ __forceinline__ int fused_sort(const PicDev& d, int s, int tid, int* s_off, int* s_cur, int* s_w)
+{
+    constexpr int PER = 256 / NT;
+    const int n_scan = d.sc_tail[s];
+    int v[PER];
+#pragma unroll
+    for (int k = 0; k < PER; ++k) {
+        v[k] = d.cell_hist_prev[(size_t)s * 256 + tid * PER + k];
+        d.cell_hist_prev[(size_t)s * 256 + tid * PER + k] = 0;
+    }
+    int total;
+    block_excl_scan256<NT>(v, total, s_w, tid);
+#pragma unroll
+    for (int k = 0; k < PER; ++k) {
+        s_off[tid * PER + k] = v[k];
+        s_cur[tid * PER + k] = v[k];
+    }
+    if (tid == 0) {
+        s_off[256] = total;
+        d.sc_count[s] = total;
+    }
+    __syncthreads();
+    if (total > n_scan || total != d.sc_next[s]) {      // histogram and records disagree: never write out of bounds
+        if (tid == 0) atomicOr(d.ctr + CTR_ERROR, PIC_DEV_SORT_MISMATCH);
+        return -1;
+    }
+    const int* tbl = d.tbl_pool + d.tbl_off[s];
+    const float4* src = d.rec[d.cur ^ 1];
+    float4* dst = d.rec[d.cur];
+    const uint32_t* sid = d.pid[d.cur ^ 1];
+    uint32_t* did = d.pid[d.cur];
+    constexpr int U = 4;               // slots per thread in flight: all loads are issued before the first use
+    for (int base = 0; base < n_scan; base += U * NT) {
+        size_t i[U];
+        float4 P[U], M[U];
+        uint32_t id[U];
+        bool ok[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int slot = base + u * NT + tid;
+            ok[u] = slot < n_scan;
+            i[u] = ok[u] ? (size_t)tbl[slot >> 8] * PIC_FRAME + (slot & (PIC_FRAME - 1)) : 0;
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+            if (ok[u]) {
+                P[u] = __ldcs(src + 2 * i[u]);
+                M[u] = __ldcs(src + 2 * i[u] + 1);
+                id[u] = __ldcs(sid + i[u]);
+            }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            if (!ok[u]) continue;
+            const uint32_t bits = __float_as_uint(M[u].w);
+            if (bits & PIC_LEFT_FLAG) continue;
+            const int r = atomicAdd(&s_cur[bits & 0xff], 1);
+            if (r >= total) {
+                atomicOr(d.ctr + CTR_ERROR, PIC_DEV_SORT_MISMATCH);
+                continue;
+            }
+            const size_t o = (size_t)tbl[r >> 8] * PIC_FRAME + (r & (PIC_FRAME - 1));
+            dst[2 * o] = P[u];
+            dst[2 * o + 1] = M[u];
+            did[o] = id[u];
+        }
+    }
+    __syncthreads();                   // the sorted records are visible to the whole CTA
+    if (tid == 0) {
+        const int keep = (total + PIC_FRAME - 1) / PIC_FRAME + 1, have = d.sc_nframes[s];
+        if (have > keep) {
+            const int at = atomicAdd(d.ctr + CTR_FREE_TOP, have - keep);
+            for (int i = keep; i < have; ++i) d.free_stack[at + i - keep] = tbl[i];
+            d.sc_nframes[s] = keep;
+        }
+    }
+    return total;
+}
+
+// Work-item order for a supercell sorted in the prologue: cells by decreasing item length (a counting sort
+// over min(length, 63); equal lengths in arrival order), first item of each.  perm/kbase as pic_sort_kernel
+// publishes them, but in shared memory.
+template <int NT>
+__device__ __forceinline__ void fused_item_order(int tid, int seg_T, const int* s_off, int* s_w, int* s_bin /*[192]*/,
+                                                 int* s_kcnt /*[256]*/, unsigned char* s_perm, unsigned short* s_kb)
+{
+    constexpr int PER = 256 / NT;
+    int* s_base = s_bin + 64;
+    int* s_bcur = s_bin + 128;
+    for (int t = tid; t < 192; t += NT) s_bin[t] = 0;
+    __syncthreads();
+    int key[PER], kk[PER];
+#pragma unroll
+    for (int k = 0; k < PER; ++k) {
+        const int c = tid * PER + k;
+        const int n = s_off[c + 1] - s_off[c];
+        kk[k] = (n + seg_T - 1) / seg_T;
+        const int seglen = kk[k] ? (n + kk[k] - 1) / kk[k] : 0;
+        key[k] = min(seglen, 63);
+        atomicAdd(&s_bin[key[k]], 1);
+    }
+    __syncthreads();
+    if (tid < 64) {
+        int b = 0;
+        for (int q = tid + 1; q < 64; ++q) b += s_bin[q];
+        s_base[tid] = b;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < PER; ++k) {
+        const int pos = s_base[key[k]] + atomicAdd(&s_bcur[key[k]], 1);
+        s_perm[pos] = (unsigned char)(tid * PER + k);
+        s_kcnt[pos] = kk[k];
+    }
+    __syncthreads();
+    int v[PER], total;
+#pragma unroll
+    for (int k = 0; k < PER; ++k) v[k] = s_kcnt[tid * PER + k];
+    block_excl_scan256<NT>(v, total, s_w, tid);
+#pragma unroll
+    for (int k = 0; k < PER; ++k) s_kb[tid * PER + k] = (unsigned short)min(v[k], 65535);
+    __syncthreads();
+}
+
 // ------------------------------------------------------------------ the step kernel
 // MODE 2: supercells with >= PIC_DIRECT_BELOW particles whose work items fit the two-phase path (<= LMAX
 //         particles each): 128 threads, per-cell stencils and Esirkepov sums in registers.
@@ -364,8 +528,13 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
     constexpr bool two_phase = MODE == PIC_MODE_TWO;
     constexpr int NT = SPARSE ? 256 : PIC_STEP_THREADS;
     {
-        const int n = d.sc_count[blockIdx.x];
-        if (n == 0 || (n < PIC_DIRECT_BELOW) != SPARSE) return;
+        // the supercell's population: after the pending sort (fused prologue), or as sorted
+        const int n = d.fused ? d.sc_next[blockIdx.x] : d.sc_count[blockIdx.x];
+        if (n == 0) {
+            if (SPARSE && d.fused && threadIdx.x == 0) d.sc_count[blockIdx.x] = 0;    // everybody left
+            return;
+        }
+        if ((n < PIC_DIRECT_BELOW) != SPARSE) return;
         if (!SPARSE) {
             const bool fits_two = d.two_phase && pic_segment_target(n, d.seg_num, PIC_ITEM_LMAX(O)) <= PIC_ITEM_LMAX(O);
             if (fits_two != two_phase) return;
@@ -423,12 +592,21 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
         }
     }
     for (int e = tid; e < NJ; e += NT) sJhi[e] = 0;
-    for (int t = tid; t < 257; t += NT) s_off[t] = d.cell_off[(size_t)s * 257 + t];
-    for (int t = tid; t < 256; t += NT) s_hist[t] = 0;
-    if constexpr (two_phase) {
-        const int nfr = (d.sc_count[s] + PIC_FRAME - 1) / PIC_FRAME;
-        if (tid < nfr) s_tbl[tid] = d.tbl_pool[d.tbl_off[s] + tid];
+    // scratch of the fused sort: the leaver staging area, unused until the particle loop
+    int* s_w = reinterpret_cast<int*>(smem_raw + S::OFF_XREC);             // [16]
+    int* s_bin = s_w + 16;                                                 // [192]
+    int* s_kcnt = s_bin + 192;                                             // [256]
+    unsigned char* s_perm = reinterpret_cast<unsigned char*>(s_kcnt + 256);       // [256]
+    unsigned short* s_kb = reinterpret_cast<unsigned short*>(s_perm + 256);       // [256]
+    static_assert((16 + 192 + 256) * 4 + 256 + 512 <= PIC_XSTAGE * 40, "sort scratch must fit the leaver staging area");
+    const bool fused = d.fused != 0;
+    if (fused) {
+        if (fused_sort<NT>(d, s, tid, s_off, s_hist, s_w) < 0) return;     // block-uniform
+        __syncthreads();
+    } else {
+        for (int t = tid; t < 257; t += NT) s_off[t] = d.cell_off[(size_t)s * 257 + t];
     }
+    for (int t = tid; t < 256; t += NT) s_hist[t] = 0;
     if (tid == 0) {
         s_xn = 0;
         s_slown = 0;
@@ -439,12 +617,17 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
     // population; cells come in the order the sort kernel fixed (by decreasing segment length), so
     // the 32 items a warp takes at a time hold similar numbers of particles
     const int seg_T = pic_segment_target(s_off[256], d.seg_num, d.two_phase ? PIC_ITEM_LMAX(O) : 0);
+    if constexpr (two_phase) {
+        const int nfr = (s_off[256] + PIC_FRAME - 1) / PIC_FRAME;
+        if (tid < nfr) s_tbl[tid] = d.tbl_pool[d.tbl_off[s] + tid];
+    }
+    if (!SPARSE && fused) fused_item_order<NT>(tid, seg_T, s_off, s_w, s_bin, s_kcnt, s_perm, s_kb);
     if (!SPARSE)
     for (int t = tid; t < 256; t += NT) {
-        const int c = d.cell_perm[(size_t)s * 256 + t];
+        const int c = fused ? s_perm[t] : d.cell_perm[(size_t)s * 256 + t];
         const int n = s_off[c + 1] - s_off[c];
         const int k = (n + seg_T - 1) / seg_T;
-        int at = d.cell_kbase[(size_t)s * 256 + t];
+        int at = fused ? s_kb[t] : d.cell_kbase[(size_t)s * 256 + t];
         if (t == 255) s_nitems = min(at + k, PIC_ITEMCAP);
         const int q = k ? n / k : 0, r = k ? n % k : 0;
         int start = s_off[c];
@@ -758,6 +941,7 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
 
     // ---- a5: leavers staged in shared memory -> one append to the exchange buffer
     const int n_x = min(s_xn, PIC_XSTAGE);
+    if (tid == 0) d.sc_left[s] = s_xn;          // every leaver, staged or appended directly (pic_prepare_kernel)
     if (tid == 0 && n_x > 0) s_xbase = atomicAdd(d.ctr + CTR_EXCH, n_x);
     __syncthreads();
     for (int k = tid; k < n_x; k += NT) {
@@ -916,6 +1100,8 @@ __global__ void pic_prepare_kernel(const PicDev d)
     }
     d.sc_tail[s] = count;
     d.sc_incoming[s] = 0;
+    d.sc_next[s] = count - d.sc_left[s] + inc;      // population after the pending sort
+    d.sc_left[s] = 0;
     atomicMax(d.ctr + CTR_MAX_COUNT, count + inc);
 }
 

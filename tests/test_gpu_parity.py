@@ -101,6 +101,35 @@ def test_gpu_continuity(name):
     pic.destroy()
 
 
+@pytest.mark.parametrize("name", ["cfg1_tiny_cic", "cfg2_thermal_tsc_32", "cfg4_khi_hotspot_tsc_24", "cfg5_pqs_32x32x16"])
+def test_one_phase_variant(name):
+    """Option two_phase=0 (gather per particle from the shared tile, DESIGN.md §5) computes the same step;
+    the default is the two-phase path (per-cell stencils in registers), covered by every other test."""
+    rep, pic, wl = _run(name, 1, two_phase=0)
+    assert rep.max_dx <= PP.TOL_X and rep.max_du_rel <= PP.TOL_U and rep.j_err_rel <= PP.TOL_J1
+    assert rep.n_member_mismatch == 0 and rep.counts_equal_outside_band
+    pic.destroy()
+
+
+@pytest.mark.parametrize("order,ppc", [(1, 40), (2, 33), (2, 40), (3, 18), (3, 30)])
+def test_item_length_limits(order, ppc):
+    """Cells that need several two-phase work items of maximal length (ppc well above the staging limit of
+    11 / 6 particles per item), and supercells just below and above the population where the item list
+    overflows and the one-phase variant takes over (768 x 11 = 8448 for CIC/TSC, 768 x 6 = 4608 for PQS)."""
+    wl = W.CONFIGS["thermal_128"].scaled((16, 16, 8), shape_order=order, ppc=ppc)
+    parts, fields = W.make_particles(wl), W.make_fields(wl)
+    orc = PP.oracle_for(wl, parts, fields)
+    pic = PP.gpu_for(wl, parts, fields)
+    assert orc.step(2) == 0
+    pic.step(2)
+    rep = PP.compare(wl, orc, pic, 2, 0.05)
+    print(f"\n[item limits order {order} ppc {ppc}] {rep}")
+    assert rep.max_dx <= 2 * PP.TOL_X and rep.max_du_rel <= 2 * PP.TOL_U and rep.j_err_rel <= 2 * PP.TOL_J1
+    assert rep.n_member_mismatch == 0 and rep.counts_equal_outside_band
+    assert pic.get_stats()["error"] == 0
+    pic.destroy()
+
+
 @pytest.mark.parametrize("order", (1, 2, 3))
 def test_fast_particles_leave_the_register_window(order):
     """c*dt = 0.9 cell and relativistic momenta: most particles move more than half a cell, leave their
