@@ -386,8 +386,9 @@ __device__ __forceinline__ void block_excl_scan256(int (&v)[256 / NT], int& tota
 // supercell: pool cur^1 (stayers, holes of leavers, appended arrivals) -> pool cur, sorted by cell.
 // Leaves the cell ranges in s_off[0..256] (shared), publishes the new count, clears the global histogram,
 // returns frames the supercell no longer needs.  s_cur: 256 ints of scratch; s_w: 16 ints of scratch.
+#define PIC_SORT_TBL 1024
 template <int NT>
-__device__ __forceinline__ int fused_sort(const PicDev& d, int s, int tid, int* s_off, int* s_cur, int* s_w)
+__device__ __forceinline__ int fused_sort(const PicDev& d, int s, int tid, int* s_off, int* s_cur, int* s_w, int* s_tbl_scr)
 {
     constexpr int PER = 256 / NT;
     const int n_scan = d.sc_tail[s];
@@ -413,34 +414,43 @@ __device__ __forceinline__ int fused_sort(const PicDev& d, int s, int tid, int* 
         if (tid == 0) atomicOr(d.ctr + CTR_ERROR, PIC_DEV_SORT_MISMATCH);
         return -1;
     }
+    // frame table in shared memory (s_tbl_scr: up to PIC_SORT_TBL entries of scratch), else straight from global
+    const int have_frames = d.sc_nframes[s];
     const int* tbl = d.tbl_pool + d.tbl_off[s];
+    if (have_frames <= PIC_SORT_TBL) {
+        for (int t = tid; t < have_frames; t += NT) s_tbl_scr[t] = tbl[t];
+        __syncthreads();
+        tbl = s_tbl_scr;
+    }
     const float4* src = d.rec[d.cur ^ 1];
     float4* dst = d.rec[d.cur];
     const uint32_t* sid = d.pid[d.cur ^ 1];
     uint32_t* did = d.pid[d.cur];
-    constexpr int U = 4;               // slots per thread in flight: all loads are issued before the first use
-    for (int base = 0; base < n_scan; base += U * NT) {
-        size_t i[U];
+    // U slots per thread and batch; the next batch is loaded while the current one is ranked and stored
+    constexpr int U = 4;
+    struct Batch {
         float4 P[U], M[U];
         uint32_t id[U];
         bool ok[U];
+    };
+    auto load = [&](Batch& q, int base) {
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             const int slot = base + u * NT + tid;
-            ok[u] = slot < n_scan;
-            i[u] = ok[u] ? (size_t)tbl[slot >> 8] * PIC_FRAME + (slot & (PIC_FRAME - 1)) : 0;
-        }
-#pragma unroll
-        for (int u = 0; u < U; ++u)
-            if (ok[u]) {
-                P[u] = __ldcs(src + 2 * i[u]);
-                M[u] = __ldcs(src + 2 * i[u] + 1);
-                id[u] = __ldcs(sid + i[u]);
+            q.ok[u] = slot < n_scan;
+            if (q.ok[u]) {
+                const size_t i = (size_t)tbl[slot >> 8] * PIC_FRAME + (slot & (PIC_FRAME - 1));
+                q.P[u] = __ldcs(src + 2 * i);
+                q.M[u] = __ldcs(src + 2 * i + 1);
+                q.id[u] = __ldcs(sid + i);
             }
+        }
+    };
+    auto place = [&](const Batch& q) {
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            if (!ok[u]) continue;
-            const uint32_t bits = __float_as_uint(M[u].w);
+            if (!q.ok[u]) continue;
+            const uint32_t bits = __float_as_uint(q.M[u].w);
             if (bits & PIC_LEFT_FLAG) continue;
             const int r = atomicAdd(&s_cur[bits & 0xff], 1);
             if (r >= total) {
@@ -448,10 +458,18 @@ __device__ __forceinline__ int fused_sort(const PicDev& d, int s, int tid, int* 
                 continue;
             }
             const size_t o = (size_t)tbl[r >> 8] * PIC_FRAME + (r & (PIC_FRAME - 1));
-            dst[2 * o] = P[u];
-            dst[2 * o + 1] = M[u];
-            did[o] = id[u];
+            dst[2 * o] = q.P[u];
+            dst[2 * o + 1] = q.M[u];
+            did[o] = q.id[u];
         }
+    };
+    Batch qa, qb;
+    load(qa, 0);
+    for (int base = 0; base < n_scan; base += 2 * U * NT) {
+        load(qb, base + U * NT);           // (slots >= n_scan: nothing is loaded)
+        place(qa);
+        load(qa, base + 2 * U * NT);
+        place(qb);
     }
     __syncthreads();                   // the sorted records are visible to the whole CTA
     if (tid == 0) {
@@ -599,9 +617,10 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
     unsigned char* s_perm = reinterpret_cast<unsigned char*>(s_kcnt + 256);       // [256]
     unsigned short* s_kb = reinterpret_cast<unsigned short*>(s_perm + 256);       // [256]
     static_assert((16 + 192 + 256) * 4 + 256 + 512 <= PIC_XSTAGE * 40, "sort scratch must fit the leaver staging area");
+    static_assert((16 + PIC_SORT_TBL) * 4 <= PIC_XSTAGE * 40, "frame table scratch must fit the leaver staging area");
     const bool fused = d.fused != 0;
     if (fused) {
-        if (fused_sort<NT>(d, s, tid, s_off, s_hist, s_w) < 0) return;     // block-uniform
+        if (fused_sort<NT>(d, s, tid, s_off, s_hist, s_w, s_w + 16) < 0) return;     // block-uniform
         __syncthreads();
     } else {
         for (int t = tid; t < 257; t += NT) s_off[t] = d.cell_off[(size_t)s * 257 + t];
