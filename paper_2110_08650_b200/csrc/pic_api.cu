@@ -417,6 +417,7 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     d.sc_tail = (int*)(w + L.sc_tail); d.sc_incoming = (int*)(w + L.sc_incoming);
     d.sc_left = (int*)(w + L.sc_left); d.sc_next = (int*)(w + L.sc_next);
     d.fused = 0;
+    d.sort_filter = 0;
     d.cell_off = (int*)(w + L.cell_off);
     c->hist[0] = (int*)(w + L.cell_hist); c->hist[1] = c->hist[0] + (size_t)L.nsc * 256;
     c->hist_cur = 0;
@@ -550,6 +551,13 @@ static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
         d.cell_hist_prev = c->hist[c->hist_cur];        // pending histogram (all zero when the state is sorted)
         c->hist_cur ^= 1;
         d.cell_hist = c->hist[c->hist_cur];             // this step's
+        if (d.fused) {      // sparse supercells: the stand-alone sort, from the other pool into this one
+            PicDev ds = d;
+            ds.cur = d.cur ^ 1;
+            ds.cell_hist = d.cell_hist_prev;
+            ds.sort_filter = 1;
+            if (e == cudaSuccess) e = pic_launch_sort(ds, st, &c->launches);
+        }
         if (e == cudaSuccess) e = pic_launch_step(d, c->order, c->use_tma && c->tmap_ok, c->fixed_point, c->tmap, st, &c->launches);
         d.fused = 0;
         if (e == cudaSuccess && c->timing) {

@@ -74,8 +74,10 @@ struct PicDev {
     int* sc_incoming;            // [nsc] leavers headed here
     int* sc_left;                // [nsc] leavers of the last step (written by the step kernel, consumed by prepare)
     int* sc_next;                // [nsc] population after the pending sort (stayers + arrivals), set by prepare
+    int sort_filter;             // pic_sort_kernel: 1 = only supercells of the sparse class (sc_next < 6 per cell)
     int fused;                   // 1: pool cur^1 holds the stepped, not yet sorted state; the step kernel sorts its
-                                 //    supercell into pool cur first, 0: pool cur is sorted
+                                 //    supercell into pool cur first (sparse supercells were sorted by
+                                 //    pic_sort_kernel just before), 0: pool cur is sorted
     // exchange buffer for supercell leavers
     float4* x_rec;               // 2 float4 per entry
     uint32_t* x_id;

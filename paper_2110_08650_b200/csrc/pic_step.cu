@@ -548,10 +548,7 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
     {
         // the supercell's population: after the pending sort (fused prologue), or as sorted
         const int n = d.fused ? d.sc_next[blockIdx.x] : d.sc_count[blockIdx.x];
-        if (n == 0) {
-            if (SPARSE && d.fused && threadIdx.x == 0) d.sc_count[blockIdx.x] = 0;    // everybody left
-            return;
-        }
+        if (n == 0) return;
         if ((n < PIC_DIRECT_BELOW) != SPARSE) return;
         if (!SPARSE) {
             const bool fits_two = d.two_phase && pic_segment_target(n, d.seg_num, PIC_ITEM_LMAX(O)) <= PIC_ITEM_LMAX(O);
@@ -618,7 +615,9 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
     unsigned short* s_kb = reinterpret_cast<unsigned short*>(s_perm + 256);       // [256]
     static_assert((16 + 192 + 256) * 4 + 256 + 512 <= PIC_XSTAGE * 40, "sort scratch must fit the leaver staging area");
     static_assert((16 + PIC_SORT_TBL) * 4 <= PIC_XSTAGE * 40, "frame table scratch must fit the leaver staging area");
-    const bool fused = d.fused != 0;
+    // sparse supercells (3 CTAs of 256 threads per SM: too few warps to hide the sort's latencies) were
+    // sorted by pic_sort_kernel just before this launch
+    const bool fused = !SPARSE && d.fused != 0;
     if (fused) {
         if (fused_sort<NT>(d, s, tid, s_off, s_hist, s_w, s_w + 16) < 0) return;     // block-uniform
         __syncthreads();
@@ -1158,6 +1157,7 @@ __global__ void __launch_bounds__(PIC_FRAME) pic_sort_kernel(const PicDev d)
     __shared__ int s_wsum[8];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int s = blockIdx.x;
+    if (d.sort_filter && d.sc_next[s] >= PIC_DIRECT_BELOW) return;     // a dense step CTA sorts this one itself
     const int n_scan = d.sc_tail[s];
     if (n_scan == 0) return;       // empty and nothing arrived: ranges, count and histogram are already zero
     const int cnt = d.cell_hist[(size_t)s * 256 + tid];
