@@ -139,8 +139,14 @@ int32_t pic_sync(pic_ctx* ctx);
  * key "tma" (1 = stage E/B tiles with cp.async.bulk.tensor, 0 = plain loads; default 1),
  * key "deposit" (1 = shared J tile accumulated in split 32-bit fixed point with native integer
  * atomics — exact, order-independent sums; 0 = float atomics, a CAS loop on sm_100a; default 1),
- * key "segment" (2..16, default 3: work-item length of the step kernel in quarters of the mean cell
- * population; set it before loading particles),
+ * key "segment" (2..16, default 3: work-item length of the one-phase step kernel in quarters of the mean
+ * cell population),
+ * key "two_phase" (1 = per-cell field stencils in registers, work items of at most 11 (PQS: 6) particles,
+ * gathered values staged in shared memory, Esirkepov sums in a second phase; 0 = gather per particle
+ * from the shared tile; default 1),
+ * key "fuse_sort" (1 = a step leaves the supercells unsorted and the next step's kernel sorts each dense
+ * supercell in its prologue; 0 = a separate sort kernel before every step; default 1),
+ * "segment" and "two_phase" fix the work-item layout the sorts publish: PIC_ESTATE once particles are loaded,
  * key "timing" (1 = record CUDA events around every launch of the step kernel, read
  * with pic_get_timing; default 0).  key is a host string. */
 int32_t pic_set_option(pic_ctx* ctx, const char* key, int64_t value);

@@ -676,10 +676,12 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
     if (!strcmp(key, "tma")) { c->use_tma = value != 0; return PIC_OK; }
     if (!strcmp(key, "graph")) { c->use_graph = value != 0; return PIC_OK; }
     if (!strcmp(key, "fuse_sort")) { c->fuse_sort = value != 0; return PIC_OK; }
-    if (!strcmp(key, "two_phase")) { c->d.two_phase = value != 0; return PIC_OK; }   // before loading particles
-    if (!strcmp(key, "segment")) {
+    if (!strcmp(key, "two_phase") || !strcmp(key, "segment")) {
+        // the sorts publish the work-item layout from these two
+        if (c->n_particles > 0) return fail(c, PIC_ESTATE, "pic_set_option: set two_phase / segment before loading particles");
+        if (key[0] == 't') { c->d.two_phase = value != 0; return PIC_OK; }
         if (value < 2 || value > 16) return fail(c, PIC_EINVAL, "pic_set_option: segment must be in 2..16");
-        c->d.seg_num = (int)value;      // takes effect at the next sort (load or step)
+        c->d.seg_num = (int)value;
         return PIC_OK;
     }
     if (!strcmp(key, "deposit")) { c->fixed_point = value != 0; return PIC_OK; }

@@ -344,6 +344,7 @@ __device__ __forceinline__ void gather_pass(const float* sF, int cx, int cy, int
         if constexpr ((MASK & 16) != 0) o[4 * NT] = st.template eval<4>(w);
         if constexpr ((MASK & 32) != 0) o[5 * NT] = st.template eval<5>(w);
     }
+    __syncwarp();       // lanes with shorter items wait here: the next phase starts converged
 }
 
 // ------------------------------------------------------------------ sort fused into the step kernel's prologue
@@ -831,6 +832,7 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
                 finish_particle(d, rec, idx, s, ssx, ssy, ssz, cx, cy, cz, sp, P, M, un, fn, sh, s_hist, &s_xn, s_xrec,
                                 s_xid, s_xdst);
             }
+            __syncwarp();
         }
         zero_sums();
         float4 Pn = stgP[0];     // {f0, q*w}
@@ -846,6 +848,7 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
             }
             deposit_in_window(f0, x1, P.w);
         }
+        __syncwarp();
     } else {
     zero_sums();
     // the next record is fetched while the current particle is processed
