@@ -111,6 +111,40 @@ def test_one_phase_variant(name):
     pic.destroy()
 
 
+@pytest.mark.parametrize("name", ["cfg2_thermal_tsc_32", "cfg3_lwfa_tsc_32x128x32", "cfg4_khi_hotspot_tsc_24"])
+def test_unfused_sort_variant(name):
+    """Option fuse_sort=0 (a separate sort kernel before every step instead of the sort in the step kernel's
+    prologue) computes the same steps."""
+    rep, pic, wl = _run(name, 3, fuse_sort=0)
+    assert rep.max_dx <= 3 * PP.TOL_X and rep.max_du_rel <= 3 * PP.TOL_U and rep.j_err_rel <= PP.TOL_J10
+    assert rep.n_member_mismatch == 0 and rep.counts_equal_outside_band
+    pic.destroy()
+
+
+def test_readbacks_between_steps_sort_the_pending_state():
+    """A step leaves the supercells unsorted (the next step's kernel sorts them).  Read-backs in between must
+    see — and leave behind — a consistent sorted state: five single steps with pic_get_counts / pic_get_particles
+    after each give bit-identical particles to one call of five steps."""
+    wl, _ = CASES["cfg2_thermal_tsc_32"]
+    parts, fields = W.make_particles(wl), W.make_fields(wl)
+    a = PP.gpu_for(wl, parts, fields)
+    b = PP.gpu_for(wl, parts, fields)
+    a.step(5)
+    for i in range(5):
+        b.step(1)
+        counts = b.get_counts()
+        assert int(counts.sum()) == parts.n
+        if i % 2 == 0:
+            assert b.get_particles()["id"].numel() == parts.n
+    A, B = PP.gpu_particles_by_id(a), PP.gpu_particles_by_id(b)
+    for k in ("x", "y", "z", "ux", "uy", "uz", "supercell"):
+        assert np.array_equal(A[k], B[k]), k
+    Ja, Jb = a.get_current().cpu().numpy(), b.get_current().cpu().numpy()
+    assert np.abs(Ja - Jb).max() <= 1e-6 * np.abs(Ja).max()      # fp32 rounding of the per-item sums (order in a cell)
+    assert torch.equal(a.get_counts(), b.get_counts())
+    a.destroy(); b.destroy()
+
+
 @pytest.mark.parametrize("order,ppc", [(1, 40), (2, 33), (2, 40), (3, 18), (3, 30)])
 def test_item_length_limits(order, ppc):
     """Cells that need several two-phase work items of maximal length (ppc well above the staging limit of
