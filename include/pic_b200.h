@@ -146,6 +146,9 @@ int32_t pic_sync(pic_ctx* ctx);
  * from the shared tile; default 1),
  * key "fuse_sort" (1 = a step leaves the supercells unsorted and the next step's kernel sorts each dense
  * supercell in its prologue; 0 = a separate sort kernel before every step; default 1),
+ * key "class_all" (-1 = decide from the population counters read at the last synchronisation which kernel
+ * variants a step launches — default; 1 = the sparse variant takes every supercell, 2 = the dense variants
+ * take every supercell, 0 = classify every supercell by its population and launch all variants),
  * "segment" and "two_phase" fix the work-item layout the sorts publish: PIC_ESTATE once particles are loaded,
  * key "timing" (1 = record CUDA events around every launch of the step kernel, read
  * with pic_get_timing; default 0).  key is a host string. */

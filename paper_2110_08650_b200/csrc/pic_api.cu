@@ -24,6 +24,8 @@ struct pic_ctx {
     bool use_tma, use_graph, fixed_point;
     bool fuse_sort;              // option "fuse_sort": the step kernel sorts its supercell first (default on)
     bool dirty;                  // pool cur holds a stepped state whose sort is still pending
+    int force_class;             // option "class_all": -1 = from the counters (default), 0/1/2 = PicDev::class_all as given
+    int max_known, min_known;    // largest / smallest non-empty supercell population as of the last synchronisation (0: unknown)
     int* hist[2];                // the two cell histograms; d.cell_hist == hist[hist_cur]
     int hist_cur;
     char* ws;
@@ -296,10 +298,14 @@ void refresh_species(pic_ctx* c)
 
 int check_device(pic_ctx* c)
 {
-    int err = 0;
-    cudaError_t e = cudaMemcpyAsync(&err, c->d.ctr + CTR_ERROR, sizeof(int), cudaMemcpyDeviceToHost, c->stream);
+    int ctr[CTR_N] = {0};
+    cudaError_t e = cudaMemcpyAsync(ctr, c->d.ctr, sizeof ctr, cudaMemcpyDeviceToHost, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "reading the device error word");
+    const int err = ctr[CTR_ERROR];
+    // populations seen so far (running max / min): lets the next steps skip kernel variants no supercell needs
+    c->max_known = ctr[CTR_MAX_COUNT];
+    c->min_known = ctr[CTR_NEGMIN] ? (1 << 30) - ctr[CTR_NEGMIN] : 0;
     if (err) {
         char buf[160];
         snprintf(buf, sizeof buf, "device fault word 0x%x (1 frame pool, 2 exchange buffer, 4 table pool, 8 moved >= 1 cell, 16 TMA timeout, 32 overflow queue, 64 sort mismatch)", err);
@@ -386,6 +392,8 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     c->use_graph = false;
     c->fuse_sort = true;
     c->dirty = false;
+    c->max_known = c->min_known = 0;
+    c->force_class = -1;
     c->fixed_point = true;
     c->tmap_ok = false;
     c->graph_exec = nullptr;
@@ -417,6 +425,7 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     d.sc_tail = (int*)(w + L.sc_tail); d.sc_incoming = (int*)(w + L.sc_incoming);
     d.sc_left = (int*)(w + L.sc_left); d.sc_next = (int*)(w + L.sc_next);
     d.fused = 0;
+    d.class_all = 0;
     d.sort_filter = 0;
     d.cell_off = (int*)(w + L.cell_off);
     c->hist[0] = (int*)(w + L.cell_hist); c->hist[1] = c->hist[0] + (size_t)L.nsc * 256;
@@ -546,16 +555,22 @@ static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
             if (e == cudaSuccess) e = cudaEventCreate(&ev1);
             if (e == cudaSuccess) e = cudaEventRecord(ev0, st);
         }
+        // which variants to launch: a belief from the last synchronisation, with a margin; a supercell that crossed
+        // the line since is still stepped correctly, by the variant that takes every supercell
+        d.class_all = 0;
+        if (c->max_known > 0 && c->max_known <= PIC_DIRECT_BELOW * 3 / 4) d.class_all = 1;
+        else if (c->min_known >= PIC_DIRECT_BELOW * 5 / 4) d.class_all = 2;
+        if (c->force_class >= 0) d.class_all = c->force_class;
         d.fused = c->dirty ? 1 : 0;
         if (c->dirty) d.cur ^= 1;       // the kernel sorts pool cur^1 into pool cur and steps it there
         d.cell_hist_prev = c->hist[c->hist_cur];        // pending histogram (all zero when the state is sorted)
         c->hist_cur ^= 1;
         d.cell_hist = c->hist[c->hist_cur];             // this step's
-        if (d.fused) {      // sparse supercells: the stand-alone sort, from the other pool into this one
+        if (d.fused && d.class_all != 2) {      // sparse supercells: the stand-alone sort, from the other pool into this one
             PicDev ds = d;
             ds.cur = d.cur ^ 1;
             ds.cell_hist = d.cell_hist_prev;
-            ds.sort_filter = 1;
+            ds.sort_filter = d.class_all == 1 ? 0 : 1;
             if (e == cudaSuccess) e = pic_launch_sort(ds, st, &c->launches);
         }
         if (e == cudaSuccess) e = pic_launch_step(d, c->order, c->use_tma && c->tmap_ok, c->fixed_point, c->tmap, st, &c->launches);
@@ -675,6 +690,11 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
     if (!c || !key) return PIC_EINVAL;
     if (!strcmp(key, "tma")) { c->use_tma = value != 0; return PIC_OK; }
     if (!strcmp(key, "graph")) { c->use_graph = value != 0; return PIC_OK; }
+    if (!strcmp(key, "class_all")) {
+        if (value < -1 || value > 2) return fail(c, PIC_EINVAL, "pic_set_option: class_all must be in -1..2");
+        c->force_class = (int)value;
+        return PIC_OK;
+    }
     if (!strcmp(key, "fuse_sort")) { c->fuse_sort = value != 0; return PIC_OK; }
     if (!strcmp(key, "two_phase") || !strcmp(key, "segment")) {
         // the sorts publish the work-item layout from these two

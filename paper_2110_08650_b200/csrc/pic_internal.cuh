@@ -35,6 +35,7 @@ enum {
     CTR_OVF = 7,
     CTR_FREE_TOP = 8,     // entries on the stack of returned frames (may dip below 0 while prepare pops)          // entries in the overflow queue of out-of-window particles (this step)
        // bits of max |weight| loaded so far (non-negative floats order like ints)
+    CTR_NEGMIN = 9,       // max over non-empty supercells of (2^30 - population) seen by pic_prepare_kernel, i.e. 2^30 - min
     CTR_N = 16
 };
 // 64-bit counters in PicDev::ctr64
@@ -74,6 +75,9 @@ struct PicDev {
     int* sc_incoming;            // [nsc] leavers headed here
     int* sc_left;                // [nsc] leavers of the last step (written by the step kernel, consumed by prepare)
     int* sc_next;                // [nsc] population after the pending sort (stayers + arrivals), set by prepare
+    int class_all;               // host's belief, from counters read at its last synchronisation (performance only, any
+                                 // value is correct): 1 = no supercell is dense: the sparse variant takes every supercell;
+                                 // 2 = none is sparse: the dense variant takes every supercell; 0 = classify by population
     int sort_filter;             // pic_sort_kernel: 1 = only supercells of the sparse class (sc_next < 6 per cell)
     int fused;                   // 1: pool cur^1 holds the stepped, not yet sorted state; the step kernel sorts its
                                  //    supercell into pool cur first (sparse supercells were sorted by
@@ -110,6 +114,7 @@ struct PicDev {
 // Two-phase path: an item's positions and gathered fields sit in shared memory, so an item holds at
 // most PIC_ITEM_LMAX particles (what fits beside the tiles with two CTAs per SM) and is flushed once.
 #define PIC_ITEM_LMAX(O) ((O) == 3 ? 6 : 11)
+#define PIC_DIRECT_BELOW 1536    // supercells with fewer particles (< 6 per cell) count as sparse: one thread per particle
 #define PIC_ITEMCAP 1024         // work items per supercell: <= 256 + count/T
 
 // Work-item length target; lmax > 0 caps it where the supercell's item list still fits PIC_ITEMCAP

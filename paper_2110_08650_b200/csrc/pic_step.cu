@@ -19,7 +19,6 @@ namespace {
 #define PIC_XSTAGE 128     // leavers staged in shared memory per CTA before one bulk append
 #define PIC_SLOWCAP_OF(O) ((O) == 3 ? 256 : 32)   // queued out-of-window particles per CTA (then: overflow queue)
 #define PIC_STEP_THREADS 128   // 2 CTAs of 4 warps per SM: ~250 registers per thread for the accumulators
-#define PIC_DIRECT_BELOW 1536   // supercells with fewer particles (< 6 per cell) take the per-particle path
 
 // Esirkepov density decomposition of one component, straight into the
 // shared tile, with a per-particle window [lo, lo+O+2):
@@ -550,7 +549,8 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
         // the supercell's population: after the pending sort (fused prologue), or as sorted
         const int n = d.fused ? d.sc_next[blockIdx.x] : d.sc_count[blockIdx.x];
         if (n == 0) return;
-        if ((n < PIC_DIRECT_BELOW) != SPARSE) return;
+        const bool sparse_class = d.class_all == 1 || (d.class_all == 0 && n < PIC_DIRECT_BELOW);
+        if (sparse_class != SPARSE) return;
         if (!SPARSE) {
             const bool fits_two = d.two_phase && pic_segment_target(n, d.seg_num, PIC_ITEM_LMAX(O)) <= PIC_ITEM_LMAX(O);
             if (fits_two != two_phase) return;
@@ -640,13 +640,16 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
         const int nfr = (s_off[256] + PIC_FRAME - 1) / PIC_FRAME;
         if (tid < nfr) s_tbl[tid] = d.tbl_pool[d.tbl_off[s] + tid];
     }
-    if (!SPARSE && fused) fused_item_order<NT>(tid, seg_T, s_off, s_w, s_bin, s_kcnt, s_perm, s_kb);
+    // the item order: published by pic_sort_kernel for the supercells it counts as dense, else worked out here
+    // (after the fused sort; or a supercell below the line that this variant takes under class_all == 2)
+    const bool own_order = fused || s_off[256] < PIC_DIRECT_BELOW;
+    if (!SPARSE && own_order) fused_item_order<NT>(tid, seg_T, s_off, s_w, s_bin, s_kcnt, s_perm, s_kb);
     if (!SPARSE)
     for (int t = tid; t < 256; t += NT) {
-        const int c = fused ? s_perm[t] : d.cell_perm[(size_t)s * 256 + t];
+        const int c = own_order ? s_perm[t] : d.cell_perm[(size_t)s * 256 + t];
         const int n = s_off[c + 1] - s_off[c];
         const int k = (n + seg_T - 1) / seg_T;
-        int at = fused ? s_kb[t] : d.cell_kbase[(size_t)s * 256 + t];
+        int at = own_order ? s_kb[t] : d.cell_kbase[(size_t)s * 256 + t];
         if (t == 255) s_nitems = min(at + k, PIC_ITEMCAP);
         const int q = k ? n / k : 0, r = k ? n % k : 0;
         int start = s_off[c];
@@ -1121,9 +1124,11 @@ __global__ void pic_prepare_kernel(const PicDev d)
     }
     d.sc_tail[s] = count;
     d.sc_incoming[s] = 0;
-    d.sc_next[s] = count - d.sc_left[s] + inc;      // population after the pending sort
+    const int next = count - d.sc_left[s] + inc;
+    d.sc_next[s] = next;                            // population after the pending sort
     d.sc_left[s] = 0;
     atomicMax(d.ctr + CTR_MAX_COUNT, count + inc);
+    if (next > 0) atomicMax(d.ctr + CTR_NEGMIN, (1 << 30) - next);
 }
 
 // One thread per leaver: claim a slot behind the destination's current slots (pool cur).
@@ -1312,13 +1317,20 @@ template <int O, bool TMA, bool FIX>
 static cudaError_t launch_step_variant(const PicDev& d, const CUtensorMap& map, cudaStream_t st, int64_t* launches)
 {
     cudaError_t e = cudaSuccess;
-    if (d.two_phase) {
-        e = launch_step_one<O, TMA, FIX, PIC_MODE_TWO>(d, map, st);
+    if (d.class_all != 1) {             // dense variants (none when the host knows every supercell to be sparse)
+        if (d.two_phase) {
+            e = launch_step_one<O, TMA, FIX, PIC_MODE_TWO>(d, map, st);
+            ++*launches;
+        }
+        if (e == cudaSuccess) {          // crowded supercells (a stale belief must not hide one) / two_phase off
+            e = launch_step_one<O, TMA, FIX, PIC_MODE_ONE>(d, map, st);
+            ++*launches;
+        }
+    }
+    if (e == cudaSuccess && d.class_all != 2) {
+        e = launch_step_one<O, TMA, FIX, PIC_MODE_SPARSE>(d, map, st);
         ++*launches;
     }
-    if (e == cudaSuccess) e = launch_step_one<O, TMA, FIX, PIC_MODE_ONE>(d, map, st);
-    if (e == cudaSuccess) e = launch_step_one<O, TMA, FIX, PIC_MODE_SPARSE>(d, map, st);
-    *launches += 2;
     return e;
 }
 

@@ -145,6 +145,19 @@ def test_readbacks_between_steps_sort_the_pending_state():
     a.destroy(); b.destroy()
 
 
+@pytest.mark.parametrize("cls", (0, 1, 2))
+@pytest.mark.parametrize("name", ["cfg3_lwfa_tsc_32x128x32", "cfg4_khi_hotspot_tsc_24", "cfg5_pqs_32x32x16"])
+def test_variant_choice_is_performance_only(name, cls):
+    """Which step-kernel variants a step launches follows the host's (possibly stale) knowledge of the supercell
+    populations; a supercell on the wrong side of the line is still stepped correctly by the variant that takes
+    every supercell.  Forced here: everything through the sparse variant (1), through the dense ones (2),
+    classified per supercell (0) — on workloads with sparse, dense and crowded supercells."""
+    rep, pic, wl = _run(name, 3, class_all=cls)
+    assert rep.max_dx <= 3 * PP.TOL_X and rep.max_du_rel <= 3 * PP.TOL_U and rep.j_err_rel <= PP.TOL_J10
+    assert rep.n_member_mismatch == 0 and rep.counts_equal_outside_band
+    pic.destroy()
+
+
 @pytest.mark.parametrize("order,ppc", [(1, 40), (2, 33), (2, 40), (3, 18), (3, 30)])
 def test_item_length_limits(order, ppc):
     """Cells that need several two-phase work items of maximal length (ppc well above the staging limit of
