@@ -106,7 +106,11 @@ int32_t pic_set_fields(pic_ctx* ctx, const float* Ex, const float* Ey, const flo
 /* Advance n steps ("pic_step(n)"); asynchronous.  Each step, per supercell:
  * stage the E/B tile + guards in shared memory, gather, Boris push, move,
  * Esirkepov deposit into a shared-memory J tile flushed once to global J, and
- * resort of particles that changed supercell. */
+ * resort of particles that changed supercell.  Leavers are
+ * moved to their new supercell within the call; the cell-order sort of every supercell
+ * is left pending and done by the next pic_step (in its kernel's prologue) or by the
+ * next call that needs the sorted arrangement (pic_load_particles, pic_get_particles,
+ * pic_get_counts) — invisible to the caller, results do not depend on it. */
 int32_t pic_step(pic_ctx* ctx, int32_t n);
 
 /* Copy the last step's J ("pic_get_current"), periodic-folded, three float32 grid
@@ -154,7 +158,8 @@ int32_t pic_sync(pic_ctx* ctx);
  * with pic_get_timing; default 0).  key is a host string. */
 int32_t pic_set_option(pic_ctx* ctx, const char* key, int64_t value);
 
-/* With option "timing": total device time in ms of the step-kernel launches since the
+/* With option "timing": total device time in ms of the step-kernel launches (including the
+ * sort of the previous step's result, which runs inside or right before them) since the
  * last call, and how many there were (host pointers, either may be NULL).  Synchronises
  * and resets the accumulation. */
 int32_t pic_get_timing(pic_ctx* ctx, double* step_kernel_ms, int64_t* step_kernel_launches);
