@@ -19,3 +19,4 @@ from .pic_oracle import (  # noqa: F401
     wrap_and_bucket,
     Oracle,
 )
+from . import yee_oracle  # noqa: F401,E402  (field update)

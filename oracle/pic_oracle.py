@@ -172,7 +172,9 @@ class Oracle:
         """fields6: array-like [6,nz,ny,nx] (Ex,Ey,Ez,Bx,By,Bz)."""
         self.fields = [_d(f) for f in fields6]
 
-    def step(self, n_steps: int = 1) -> int:
+    def step(self, n_steps: int = 1, update_fields: bool = False) -> int:
+        """update_fields: after every particle step advance E, B with that step's J
+        (oracle/yee_oracle.py) — the self-consistent PIC loop."""
         rc = 0
         x, y, z, ux, uy, uz, w = self._parts
         for _ in range(n_steps):
@@ -180,7 +182,16 @@ class Oracle:
                 j.fill(0.0)                       # S16: J is the last step's current
             rc |= step(self.prm, x, y, z, ux, uy, uz, w, self.species, self.q, self.m,
                        self.fields, self.J, self.supercell)
+            if update_fields:
+                self.update_fields()
         return rc
+
+    def update_fields(self):
+        """One Yee update of the fields with the last step's J."""
+        from . import yee_oracle
+        p = self.prm
+        self.fields = [np.ascontiguousarray(f) for f in
+                       yee_oracle.yee_update(self.fields, self.J, p.dt, (p.dx, p.dy, p.dz))]
 
     def particles(self):
         x, y, z, ux, uy, uz, w = self._parts

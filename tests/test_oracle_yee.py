@@ -1,0 +1,161 @@
+"""Pins of oracle/yee_oracle.py to what the mathematics fixes — none of them
+retypes the oracle's difference expressions:
+
+* a discrete plane wave with the scheme's numerical dispersion relation is an EXACT solution
+  (closed form below, derived by hand), for oblique k, anisotropic cells, all polarisations;
+* div B is conserved identically, Gauss's law follows the Esirkepov current of the particle
+  oracle (end-to-end: deposit + field update), both to round-off;
+* a uniform J is a pure impulse on E; the curl of a discrete gradient vanishes.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from oracle import yee_oracle as Y
+
+STAG = {"Ex": (0.5, 0, 0), "Ey": (0, 0.5, 0), "Ez": (0, 0, 0.5),
+        "Bx": (0, 0.5, 0.5), "By": (0.5, 0, 0.5), "Bz": (0.5, 0.5, 0)}
+
+
+def _plane_wave(grid, cell, dt, modes, pol_seed):
+    """Closed form.  With K_a = (2/dx_a) sin(k_a dx_a/2) a centred difference of
+    cos(k.r - w t) equals -K_a sin(k.r - w t) at the midpoint, and (2/dt) sin(w dt/2) =: W
+    plays the same role in time.  Faraday and Ampere then read W B0 = K x E0, W E0 = -K x B0:
+    K.E0 = 0 and W = |K| (the numerical dispersion relation).  B at integer time levels is the
+    mean of the two neighbouring half levels = B0 cos(w dt/2) cos(k.r - w t_n)."""
+    nx, ny, nz = grid
+    k = np.array([2 * math.pi * m / (n * d) for m, n, d in zip(modes, grid, cell)])
+    K = np.array([2.0 / d * math.sin(ka * d / 2) for ka, d in zip(k, cell)])
+    Kn = np.linalg.norm(K)
+    assert dt * Kn / 2 < 1, "CFL"
+    w = 2.0 / dt * math.asin(dt * Kn / 2)
+    rng = np.random.default_rng(pol_seed)
+    v = rng.normal(size=3)
+    E0 = v - K * (K @ v) / (K @ K)           # discretely transverse
+    B0 = np.cross(K, E0) / Kn
+
+    def component(name, amp, t):
+        s = STAG[name]
+        z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+        ph = k[0] * (x + s[0]) * cell[0] + k[1] * (y + s[1]) * cell[1] + k[2] * (z + s[2]) * cell[2]
+        return amp * np.cos(ph - w * t)
+
+    def at(n):
+        t = n * dt
+        c = math.cos(w * dt / 2)
+        return [component("Ex", E0[0], t), component("Ey", E0[1], t), component("Ez", E0[2], t),
+                component("Bx", B0[0] * c, t), component("By", B0[1] * c, t), component("Bz", B0[2] * c, t)]
+
+    return at, w
+
+
+@pytest.mark.parametrize("modes,cell,dt", [((1, 0, 0), (1.0, 1.0, 1.0), 0.5),
+                                           ((0, 2, 0), (1.0, 1.0, 1.0), 0.5),
+                                           ((0, 0, 1), (1.0, 1.0, 1.0), 0.5),
+                                           ((2, -1, 3), (1.0, 1.0, 1.0), 0.5),
+                                           ((1, 2, -1), (0.8, 1.25, 1.5), 0.4)])
+def test_discrete_plane_wave_is_exact(modes, cell, dt):
+    grid = (16, 12, 8)
+    at, w = _plane_wave(grid, cell, dt, modes, pol_seed=7)
+    F = at(0)
+    zero = [np.zeros_like(F[0])] * 3
+    scale = max(np.abs(f).max() for f in F)
+    for n in range(1, 41):
+        F = Y.yee_update(F, zero, dt, cell)
+        if n in (1, 7, 40):
+            for got, exp in zip(F, at(n)):
+                assert np.abs(got - exp).max() < 1e-12 * scale
+
+
+def test_numerical_phase_velocity_is_below_c_and_second_order():
+    """w from the dispersion relation the wave test uses, against the continuum w = |k|:
+    relative lag ~ (k dx)^2/24 (1 - (dt/dx)^2) for a wave along one axis."""
+    lags = []
+    for n in (16, 32, 64):
+        _, w = _plane_wave((n, 8, 8), (1.0, 1.0, 1.0), 0.5, (1, 0, 0), 1)
+        k = 2 * math.pi / n
+        lags.append(1 - w / k)
+        assert 0 < lags[-1]
+        assert lags[-1] == pytest.approx(k * k / 24 * (1 - 0.25), rel=0.05)
+    assert lags[0] / lags[1] == pytest.approx(4, rel=0.02) and lags[1] / lags[2] == pytest.approx(4, rel=0.02)
+
+
+def test_div_B_conserved_and_uniform_J_impulse():
+    rng = np.random.default_rng(3)
+    shp = (8, 12, 16)
+    cell = (1.0, 0.7, 1.3)
+    F = [rng.normal(size=shp) for _ in range(6)]
+    J = [rng.normal(size=shp) for _ in range(3)]
+    d0 = Y.div_B(*F[3:], cell)
+    G = Y.yee_update(F, J, 0.3, cell)
+    assert np.abs(Y.div_B(*G[3:], cell) - d0).max() < 1e-13 * np.abs(d0).max()
+    # uniform fields, uniform J: E changes by -dt*J exactly, B stays
+    F = [np.full(shp, v) for v in (0.1, -0.2, 0.3, 0.4, 0.5, -0.6)]
+    J = [np.full(shp, v) for v in (1.0, 2.0, -3.0)]
+    G = Y.yee_update(F, J, 0.25, cell)
+    for a, (e0, j) in enumerate(zip((0.1, -0.2, 0.3), (1.0, 2.0, -3.0))):
+        assert np.abs(G[a] - (e0 - 0.25 * j)).max() < 1e-15
+    for a, b0 in enumerate((0.4, 0.5, -0.6)):
+        assert np.abs(G[3 + a] - b0).max() < 1e-15
+
+
+def test_curl_of_discrete_gradient_vanishes():
+    """E = -grad(phi) built with plain index arithmetic (Ex[i] = -(phi[i+1]-phi[i])/dx at i+1/2):
+    Faraday leaves B untouched."""
+    rng = np.random.default_rng(5)
+    nz, ny, nx = 6, 8, 10
+    cell = (1.1, 0.9, 1.4)
+    phi = rng.normal(size=(nz, ny, nx))
+    Ex = np.empty_like(phi); Ey = np.empty_like(phi); Ez = np.empty_like(phi)
+    for k in range(nz):
+        for j in range(ny):
+            for i in range(nx):
+                Ex[k, j, i] = -(phi[k, j, (i + 1) % nx] - phi[k, j, i]) / cell[0]
+                Ey[k, j, i] = -(phi[k, (j + 1) % ny, i] - phi[k, j, i]) / cell[1]
+                Ez[k, j, i] = -(phi[(k + 1) % nz, j, i] - phi[k, j, i]) / cell[2]
+    c = Y.curl_E(Ex, Ey, Ez, cell)
+    assert max(np.abs(a).max() for a in c) < 1e-13 * np.abs(Ex).max()
+
+
+@pytest.mark.parametrize("order", (1, 2, 3))
+def test_gauss_law_follows_the_esirkepov_current(order):
+    """End to end with the particle oracle: div E^{n+1} - rho^{n+1} = div E^n - rho^n at every
+    node, because Esirkepov's J satisfies the discrete continuity equation with the same
+    backward divergence.  rho is computed by brute force below (plain loops over the shape's
+    support with scipy's B-spline), not by the oracle."""
+    from conftest import bspline_ref
+    rng = np.random.default_rng(11)
+    grid, cell, dt = (8, 8, 8), (1.0, 1.0, 1.0), 0.5
+    n = 40
+    orc = oracle.Oracle(grid, cell, dt, (8, 8, 4), order)
+    x, y, z = (rng.uniform(0, g, n) for g in grid)
+    u = rng.normal(scale=0.5, size=(3, n))
+    w = rng.uniform(0.5, 1.5, n)
+    sp = rng.integers(0, 2, n).astype(np.int32)
+    orc.set_species([-1.0, 2.0], [1.0, 3.0])
+    orc.load_particles(x, y, z, u[0], u[1], u[2], w, sp)
+    orc.set_fields([rng.normal(scale=0.05, size=(8, 8, 8)) for _ in range(6)])
+
+    def rho_brute():
+        P = orc.particles()
+        r = np.zeros((8, 8, 8))
+        qw = orc.q[orc.species] * P["w"]
+        for p in range(n):
+            X = (P["x"][p], P["y"][p], P["z"][p])
+            base = [int(math.floor(c)) for c in X]
+            for dk in range(-2, 4):
+                for dj in range(-2, 4):
+                    for di in range(-2, 4):
+                        i, j, k = base[0] + di, base[1] + dj, base[2] + dk
+                        wgt = (bspline_ref(order, X[0] - i) * bspline_ref(order, X[1] - j)
+                               * bspline_ref(order, X[2] - k))
+                        r[k % 8, j % 8, i % 8] += qw[p] * float(wgt)
+        return r
+
+    g0 = Y.div_E(*orc.fields[:3], cell) - rho_brute()
+    for _ in range(3):
+        assert orc.step(1, update_fields=True) == 0
+    g1 = Y.div_E(*orc.fields[:3], cell) - rho_brute()
+    assert np.abs(g1 - g0).max() < 1e-12 * max(1.0, np.abs(g0).max())
