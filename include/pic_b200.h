@@ -98,8 +98,9 @@ int32_t pic_load_particles(pic_ctx* ctx, int64_t n,
                            const float* ux, const float* uy, const float* uz,
                            const float* w, const int32_t* species);
 
-/* Set the static external fields ("pic_set_fields(E,B)"): six float32 grid arrays,
- * copied into the workspace (asynchronous). */
+/* Set the fields ("pic_set_fields(E,B)"): six float32 grid arrays, copied into the workspace
+ * (asynchronous).  They stay as set (static external fields, the contract's five configs) unless
+ * pic_update_fields / option "field_update" advances them. */
 int32_t pic_set_fields(pic_ctx* ctx, const float* Ex, const float* Ey, const float* Ez,
                        const float* Bx, const float* By, const float* Bz);
 
@@ -112,6 +113,21 @@ int32_t pic_set_fields(pic_ctx* ctx, const float* Ex, const float* Ey, const flo
  * next call that needs the sorted arrangement (pic_load_particles, pic_get_particles,
  * pic_get_counts) — invisible to the caller, results do not depend on it. */
 int32_t pic_step(pic_ctx* ctx, int32_t n);
+
+/* One Yee update of E and B with the last step's J, closing the PIC loop (PAPER.md:60
+ * "fields generated by moving particles"; c = eps0 = mu0 = 1, periodic):
+ *     B^{n+1/2} = B^n - (dt/2) curl E^n;   E^{n+1} = E^n + dt (curl B^{n+1/2} - J);
+ *     B^{n+1} = B^{n+1/2} - (dt/2) curl E^{n+1},
+ * curl E by forward differences onto the B locations, curl B by backward differences onto the E
+ * locations.  E and B are both kept at the integer time level the particle step gathers at; J is
+ * whatever pic_get_current would return (zero before the first step).  After pic_step(1) this
+ * advances the fields consistently with the particles; with option "field_update" = 1 every step of
+ * pic_step(n) ends with it.  Asynchronous; PIC_ESTATE before pic_set_fields. */
+int32_t pic_update_fields(pic_ctx* ctx);
+
+/* Copy the current E, B out: six float32 grid arrays (any may be NULL).  Asynchronous
+ * device-to-device copies on the stream; PIC_ESTATE before pic_set_fields. */
+int32_t pic_get_fields(pic_ctx* ctx, float* Ex, float* Ey, float* Ez, float* Bx, float* By, float* Bz);
 
 /* Copy the last step's J ("pic_get_current"), periodic-folded, three float32 grid
  * arrays (any may be NULL).  Asynchronous device-to-device copy on the stream. */
@@ -150,6 +166,7 @@ int32_t pic_sync(pic_ctx* ctx);
  * from the shared tile; default 1),
  * key "fuse_sort" (1 = a step leaves the supercells unsorted and the next step's kernel sorts each dense
  * supercell in its prologue; 0 = a separate sort kernel before every step; default 1),
+ * key "field_update" (1 = every step of pic_step ends with pic_update_fields: the self-consistent loop; default 0),
  * key "class_all" (-1 = decide from the population counters read at the last synchronisation which kernel
  * variants a step launches — default; 1 = the sparse variant takes every supercell, 2 = the dense variants
  * take every supercell, 0 = classify every supercell by its population and launch all variants),

@@ -23,6 +23,7 @@ SYMBOLS = (
     "pic_workspace_bytes", "pic_create", "pic_set_species", "pic_load_particles", "pic_set_fields",
     "pic_step", "pic_get_current", "pic_get_particles", "pic_get_counts", "pic_get_stats", "pic_sync",
     "pic_set_option", "pic_get_timing", "pic_launch_count", "pic_last_error", "pic_destroy",
+    "pic_update_fields", "pic_get_fields",
 )
 
 
@@ -67,6 +68,8 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     L.pic_last_error.argtypes = [vp]
     L.pic_last_error.restype = C.c_char_p
     L.pic_destroy.argtypes = [vp]
+    L.pic_update_fields.argtypes = [vp]
+    L.pic_get_fields.argtypes = [vp] + [vp] * 6
     for name in SYMBOLS:
         if name not in ("pic_launch_count", "pic_last_error"):
             getattr(L, name).restype = i32
@@ -169,6 +172,18 @@ class Pic:
 
     def step(self, n: int = 1):
         self._check(self._L.pic_step(self._h, int(n)))
+
+    def update_fields(self):
+        """One Yee update of E, B with the last step's J (pic_update_fields)."""
+        self._check(self._L.pic_update_fields(self._h))
+
+    def get_fields(self) -> torch.Tensor:
+        """float32 [6, nz, ny, nx]: the current Ex,Ey,Ez,Bx,By,Bz."""
+        nx, ny, nz = self.grid
+        F = torch.empty((6, nz, ny, nx), dtype=torch.float32, device=self.device)
+        nb = self.n_cells * 4
+        self._check(self._L.pic_get_fields(self._h, *[C.c_void_p(F.data_ptr() + c * nb) for c in range(6)]))
+        return F
 
     def get_current(self) -> torch.Tensor:
         """float32 [3, nz, ny, nx]: J of the last step."""

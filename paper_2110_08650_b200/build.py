@@ -14,11 +14,11 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpic_b200.so")
-SOURCES = ("pic_api.cu", "pic_step.cu")
+SOURCES = ("pic_api.cu", "pic_step.cu", "pic_fields.cu")
 HEADERS = ("pic_internal.cuh", "pic_device.cuh", os.path.join("..", "..", "include", "pic_b200.h"))
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-    "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "--use_fast_math=false",
+    "-Xcompiler", "-fPIC", "-cudart", "static",
 ]
 
 
@@ -37,24 +37,41 @@ def _stale() -> bool:
     return any(os.path.getmtime(p) > t for p in deps)
 
 
-def build_library(force: bool = False, verbose: bool = False) -> str:
-    """Compile the CUDA sources into libpic_b200.so if missing or out of date."""
-    if not force and not _stale():
-        return LIB
-    tmp = LIB + f".tmp{os.getpid()}"
-    flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
-    cmd = [_nvcc(), *flags, "-o", tmp, *[os.path.join(CSRC, s) for s in SOURCES]]
-    if verbose:
-        cmd.insert(1, "-Xptxas")
-        cmd.insert(2, "-v")
+def _run(cmd, verbose: bool):
     res = subprocess.run(cmd, capture_output=True, text=True)
     if res.returncode != 0:
-        if os.path.exists(tmp):
-            os.remove(tmp)
         raise RuntimeError("nvcc failed:\n" + res.stdout + res.stderr)
     if verbose:
         sys.stderr.write(res.stdout + res.stderr)
-    os.replace(tmp, LIB)
+
+
+def build_library(force: bool = False, verbose: bool = False) -> str:
+    """Compile the CUDA sources into libpic_b200.so if missing or out of date: one object per source
+    (rebuilt when the source, a header or this script is newer), then one link."""
+    if not force and not _stale():
+        return LIB
+    hdr_t = max(os.path.getmtime(os.path.join(CSRC, h)) for h in HEADERS)
+    hdr_t = max(hdr_t, os.path.getmtime(os.path.abspath(__file__)))
+    objs = []
+    for s in SOURCES:
+        src = os.path.join(CSRC, s)
+        obj = os.path.join(CSRC, s[:-3] + ".o")
+        objs.append(obj)
+        if force or not os.path.exists(obj) or os.path.getmtime(obj) < max(hdr_t, os.path.getmtime(src)):
+            tmp = obj + f".tmp{os.getpid()}"
+            try:
+                _run([_nvcc(), *(["-Xptxas", "-v"] if verbose else []), *NVCC_FLAGS, "-c", "-o", tmp, src], verbose)
+                os.replace(tmp, obj)
+            finally:
+                if os.path.exists(tmp):
+                    os.remove(tmp)
+    tmp = LIB + f".tmp{os.getpid()}"
+    try:
+        _run([_nvcc(), *NVCC_FLAGS, "-shared", "-o", tmp, *objs], verbose)
+        os.replace(tmp, LIB)
+    finally:
+        if os.path.exists(tmp):
+            os.remove(tmp)
     return LIB
 
 

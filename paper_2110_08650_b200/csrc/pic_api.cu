@@ -23,6 +23,9 @@ struct pic_ctx {
     bool have_fields;
     bool use_tma, use_graph, fixed_point;
     bool fuse_sort;              // option "fuse_sort": the step kernel sorts its supercell first (default on)
+    bool field_update;           // option "field_update": every step ends with a Yee update of E, B (pic_fields.cu)
+    float* Fbuf[2];              // the two plain field buffers; d.F == Fbuf[F_cur]
+    int F_cur;
     bool dirty;                  // pool cur holds a stepped state whose sort is still pending
     int force_class;             // option "class_all": -1 = from the counters (default), 0/1/2 = PicDev::class_all as given
     int max_known, min_known;    // largest / smallest non-empty supercell population as of the last synchronisation (0: unknown)
@@ -48,7 +51,7 @@ namespace {
 
 struct Layout {
     uint64_t rec0, rec1, pid0, pid1, free_stack, tbl_pool, tbl_off, tbl_cap, sc_nframes, sc_count, sc_tail, sc_incoming,
-        sc_left, sc_next, cell_off, cell_hist, cell_perm, cell_kbase, x_rec, x_id, x_dst, ovf, ctr, ctr64, F, Fpad, J, J64, sc_offset, total;
+        sc_left, sc_next, cell_off, cell_hist, cell_perm, cell_kbase, x_rec, x_id, x_dst, ovf, ctr, ctr64, F, F2, Fpad, J, J64, sc_offset, total;
     int n_frames, tbl_pool_size, x_cap, nsc;
 };
 
@@ -98,6 +101,7 @@ int compute_layout(const int32_t grid[3], const int32_t sc[3], int order, int64_
     L->ctr = take(CTR_N * 4);
     L->ctr64 = take(CTR64_N * 8);
     L->F = take(6 * ncell * 4);
+    L->F2 = take(6 * ncell * 4);                 // second field buffer of the Yee update (pic_fields.cu)
     L->Fpad = take(6ull * (grid[0] + PIC_PAD_X) * (grid[1] + PIC_PAD_Y) * (grid[2] + PIC_PAD_Z) * 4);
     L->J = take(3 * ncell * 4);
     L->J64 = take(3 * ncell * 8);
@@ -391,6 +395,7 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     c->use_tma = true;
     c->use_graph = false;
     c->fuse_sort = true;
+    c->field_update = false;
     c->dirty = false;
     c->max_known = c->min_known = 0;
     c->force_class = -1;
@@ -437,6 +442,7 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     d.ovf = (float4*)(w + L.ovf); d.ovf_cap = L.x_cap;
     d.x_id = (uint32_t*)(w + L.x_id); d.x_dst = (int*)(w + L.x_dst); d.x_cap = L.x_cap;
     d.ctr = (int*)(w + L.ctr); d.ctr64 = (unsigned long long*)(w + L.ctr64);
+    c->Fbuf[0] = (float*)(w + L.F); c->Fbuf[1] = (float*)(w + L.F2); c->F_cur = 0;
     d.F = (const float*)(w + L.F); d.Fpad = (const float*)(w + L.Fpad); d.J = (float*)(w + L.J); d.J64 = (long long*)(w + L.J64);
     d.sc_offset = (long long*)(w + L.sc_offset);
     d.pad_lo_x = (shape_order == 3) ? 2 : 1;
@@ -533,6 +539,16 @@ static int ensure_sorted(pic_ctx* c)
     return PIC_OK;
 }
 
+// One Yee update with the last step's J: level n in Fbuf[F_cur] -> level n+1 in the other buffer and in Fpad.
+static cudaError_t enqueue_field_update(pic_ctx* c, cudaStream_t st)
+{
+    cudaError_t e = pic_launch_yee(c->d, c->Fbuf[c->F_cur], c->Fbuf[c->F_cur ^ 1], c->dt, c->cell, st, &c->launches);
+    if (e != cudaSuccess) return e;
+    c->F_cur ^= 1;
+    c->d.F = c->Fbuf[c->F_cur];
+    return cudaSuccess;
+}
+
 // One step = [sort of the previous step's result, fused into the step kernel's prologue] + gather, push,
 // deposit, in-place write-back + convert J + make room + scatter leavers.  The state is left unsorted
 // ("dirty"); whoever needs the sorted arrangement (the next step, a load, a read-back) sorts it.
@@ -584,6 +600,7 @@ static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
         if (e == cudaSuccess && c->fixed_point) e = pic_launch_convert(d, st, &c->launches);
         if (e == cudaSuccess) e = pic_launch_prepare(d, st, &c->launches);
         if (e == cudaSuccess) e = pic_launch_scatter(d, st, &c->launches);
+        if (e == cudaSuccess && c->field_update) e = enqueue_field_update(c, st);
         if (e != cudaSuccess) return cuda_fail(c, e, "pic_step: launch");
         c->dirty = true;
     }
@@ -599,6 +616,30 @@ int32_t pic_step(pic_ctx* c, int32_t n)
     int rc = enqueue_steps(c, n, c->stream);
     if (rc == PIC_OK) c->steps += n;
     return rc;
+}
+
+int32_t pic_update_fields(pic_ctx* c)
+{
+    if (!c) return PIC_EINVAL;
+    if (!c->have_fields) return fail(c, PIC_ESTATE, "pic_update_fields: pic_set_fields has not been called");
+    cudaError_t e = enqueue_field_update(c, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "pic_update_fields: launch");
+    return PIC_OK;
+}
+
+int32_t pic_get_fields(pic_ctx* c, float* Ex, float* Ey, float* Ez, float* Bx, float* By, float* Bz)
+{
+    if (!c) return PIC_EINVAL;
+    if (!c->have_fields) return fail(c, PIC_ESTATE, "pic_get_fields: pic_set_fields has not been called");
+    float* dst[6] = {Ex, Ey, Ez, Bx, By, Bz};
+    const size_t ncell = (size_t)c->d.nx * c->d.ny * c->d.nz;
+    for (int k = 0; k < 6; ++k) {
+        if (!dst[k]) continue;
+        cudaError_t e = cudaMemcpyAsync(dst[k], c->d.F + k * ncell, ncell * sizeof(float),
+                                        cudaMemcpyDeviceToDevice, c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e, "pic_get_fields: cudaMemcpyAsync");
+    }
+    return PIC_OK;
 }
 
 int32_t pic_get_current(pic_ctx* c, float* Jx, float* Jy, float* Jz)
@@ -696,6 +737,7 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
         return PIC_OK;
     }
     if (!strcmp(key, "fuse_sort")) { c->fuse_sort = value != 0; return PIC_OK; }
+    if (!strcmp(key, "field_update")) { c->field_update = value != 0; return PIC_OK; }
     if (!strcmp(key, "two_phase") || !strcmp(key, "segment")) {
         // the sorts publish the work-item layout from these two
         if (c->n_particles > 0) return fail(c, PIC_ESTATE, "pic_set_option: set two_phase / segment before loading particles");

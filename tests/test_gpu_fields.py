@@ -1,0 +1,142 @@
+"""CUDA-vs-oracle parity of the Yee field update (pic_update_fields) and of the
+self-consistent loop (option field_update), through the C ABI.
+
+Tolerance of the fields: one update rounds E + dt*(curl B - J) and twice B - dt/2*curl E
+in fp32 — a handful of half-ulp errors of max|F| each — and the scheme does not amplify them, so after n
+updates |F_gpu - F_oracle| <= n * 1e-6 * max(|E|, |B|, dt*|J|) (measured: ~1.5e-7 per update).
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import pic_parity as PP
+from oracle import yee_oracle as Y
+from paper_2110_08650_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_F = 1e-6
+
+
+def _vacuum(grid, order):
+    from paper_2110_08650_b200.binding import Pic
+    wl = W.CONFIGS["thermal_128"].scaled(grid, shape_order=order)
+    return wl, Pic(wl.grid, wl.cell, wl.dt, wl.supercell, wl.shape_order, max_particles=0)
+
+
+@pytest.mark.parametrize("grid", [(16, 16, 8), (40, 24, 20), (64, 16, 12), (8, 8, 4)])
+@pytest.mark.parametrize("order", (2, 3))
+def test_vacuum_update_matches_oracle(grid, order):
+    """No particles (J = 0): grids smaller than one 32x8x8 tile, ragged tiles, several tiles."""
+    wl, pic = _vacuum(grid, order)
+    F0 = W.make_fields(wl)
+    pic.set_fields(F0.cuda().contiguous())
+    F = [f.astype(np.float64) for f in F0.numpy()]
+    zero = [np.zeros_like(F[0])] * 3
+    scale = max(np.abs(f).max() for f in F)
+    for n in range(1, 6):
+        pic.update_fields()
+        F = Y.yee_update(F, zero, wl.dt, wl.cell)
+        G = pic.get_fields().cpu().numpy().astype(np.float64)
+        err = np.abs(G - np.stack(F)).max()
+        assert err <= n * TOL_F * scale, (n, err / scale)
+    pic.sync()
+    pic.destroy()
+
+
+def test_plane_wave_against_the_closed_form():
+    """40 updates of a discrete plane wave (oblique k) against the analytic solution with the numerical
+    dispersion relation (derivation: tests/test_oracle_yee.py) — no oracle involved."""
+    from test_oracle_yee import _plane_wave
+    grid = (32, 16, 8)
+    wl, pic = _vacuum(grid, 2)
+    at, w = _plane_wave(grid, wl.cell, wl.dt, (2, -1, 1), pol_seed=3)
+    F0 = np.stack(at(0))
+    scale = np.abs(F0).max()
+    pic.set_fields(torch.from_numpy(F0.astype(np.float32)).cuda().contiguous())
+    for n in range(1, 41):
+        pic.update_fields()
+    G = pic.get_fields().cpu().numpy().astype(np.float64)
+    err = np.abs(G - np.stack(at(40))).max()
+    print(f"\n[plane wave, 40 updates] err/max|F| = {err / scale:.3e}")
+    # the initial state itself is rounded to fp32 (6e-8 relative), then 40 updates
+    assert err <= 41 * TOL_F * scale
+    pic.destroy()
+
+
+def _loop_case(order, grid=(24, 16, 12), ppc=8, weight=0.01):
+    wl = W.CONFIGS["thermal_128"].scaled(grid, shape_order=order, ppc=ppc)
+    parts, fields = W.make_particles(wl), W.make_fields(wl)
+    parts.w.mul_(weight)       # omega_p*dt = sqrt(ppc*w)*dt = 0.14: a stable, weakly coupled plasma
+    return wl, parts, fields
+
+
+@pytest.mark.parametrize("order", (1, 2, 3))
+@pytest.mark.parametrize("mode", ("option_tma", "option_plain_loads", "explicit_calls"))
+def test_self_consistent_loop(order, mode):
+    """Ten steps of push + deposit + field update on both sides, free-running."""
+    n_steps = 10
+    wl, parts, fields = _loop_case(order)
+    orc = PP.oracle_for(wl, parts, fields)
+    opts = {"tma": 0} if mode == "option_plain_loads" else {}
+    pic = PP.gpu_for(wl, parts, fields, **opts)
+    assert orc.step(n_steps, update_fields=True) == 0
+    if mode == "explicit_calls":
+        for _ in range(n_steps):
+            pic.step(1)
+            pic.update_fields()
+    else:
+        pic.set_option("field_update", 1)
+        pic.step(n_steps)
+    pic.sync()
+    rep = PP.compare(wl, orc, pic, n_steps, 0.05)
+    G = pic.get_fields().cpu().numpy().astype(np.float64)
+    Fo = np.stack(orc.fields)
+    scale = np.abs(Fo).max()
+    f_err = np.abs(G - Fo).max() / scale
+    print(f"\n[loop order={order} {mode}] {rep}  fields err/max|F|={f_err:.3e}")
+    assert rep.max_dx <= n_steps * PP.TOL_X and rep.max_du_rel <= n_steps * PP.TOL_U
+    assert rep.j_err_rel <= PP.TOL_J10
+    assert rep.n_member_mismatch == 0 and rep.counts_equal_outside_band
+    assert f_err <= n_steps * TOL_F
+    # the fields did change: this is not the static-field path
+    assert np.abs(Fo - fields.numpy()).max() > 0.05 * scale
+    pic.destroy()
+
+
+@pytest.mark.parametrize("order", (2, 3))
+def test_gauss_law_is_kept_on_the_gpu(order):
+    """div E - rho at the nodes stays what it was: the GPU's Esirkepov J and its field update use the same
+    discrete divergence.  rho in fp64 from the GPU's own positions (S22's recipe)."""
+    wl, parts, fields = _loop_case(order)
+    pic = PP.gpu_for(wl, parts, fields, field_update=1)
+    prm = oracle.OracleParams.make(wl.grid, wl.cell, wl.dt, wl.supercell, wl.shape_order)
+
+    def gauss():
+        P = PP.gpu_particles_by_id(pic)
+        rho = oracle.rho(prm, P["x"], P["y"], P["z"], -P["w"].astype(np.float64))
+        E = pic.get_fields().cpu().numpy().astype(np.float64)[:3]
+        return Y.div_E(*E, wl.cell) - rho, np.abs(rho).max()
+
+    g0, rmax = gauss()
+    n_steps = 5
+    pic.step(n_steps)
+    pic.sync()
+    g1, _ = gauss()
+    drift = np.abs(g1 - g0).max() / rmax
+    print(f"\n[gauss order={order}] drift of (div E - rho) / max|rho| after {n_steps} steps = {drift:.3e}")
+    assert drift <= n_steps * PP.TOL_CONT
+    pic.destroy()
+
+
+def test_update_before_set_fields_is_a_state_error():
+    from paper_2110_08650_b200.binding import Pic, PicError
+    pic = Pic((16, 16, 8), shape_order=1, max_particles=0)
+    with pytest.raises(PicError):
+        pic.update_fields()
+    with pytest.raises(PicError):
+        pic.get_fields()
+    pic.destroy()
