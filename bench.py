@@ -32,6 +32,9 @@ UNIT = "particle-steps/s"
 PARTICLE_BYTES = 64.0      # float4 pos + float4 mom, read + write (SURVEY.md §8(d), 64 B basis)
 GRID_BYTES_PER_CELL = 36.0  # E+B read once (24 B) + J written once (12 B) per cell per step
 LEAVER_BYTES = 36.0 * 0.015
+# Yee update: E, B, J read once (36 B), E, B written once (24 B) and once more into the padded
+# copy the step kernel's TMA reads (24 B)
+FIELD_UPDATE_BYTES_PER_CELL = 84.0
 
 
 def algorithmic_bytes_per_particle_step(wl, n_particles: int) -> float:
@@ -245,6 +248,7 @@ def run_ours(args):
         pic.set_option("deposit", args.deposit)
         pic.set_option("segment", args.segment)
         pic.set_option("two_phase", args.two_phase)
+        pic.set_option("field_update", args.self_consistent)
         return pic
 
     # ---------------------------------------------------------------- device-resident throughput
@@ -276,6 +280,29 @@ def run_ours(args):
     stats = pic.get_stats()
     ms_max, kernel_ms_avg = reduce_max_over_ranks([ms, kernel_ms / max(n_kernel, 1)], dev, world)
     value = whole_job_value(world, n, K, ms_max * 1e-3)
+
+    # ---------------------------------------------------------------- the Yee field update alone
+    fu = None
+    if args.field_update_reps > 0 and rank == 0:
+        R = args.field_update_reps
+        for _ in range(3):
+            pic.update_fields()
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        f0.record(pic.stream)
+        for _ in range(R):
+            pic.update_fields()
+        f1.record(pic.stream)
+        torch.cuda.synchronize()
+        fu_ms = f0.elapsed_time(f1) / R
+        peak_f, _ = measured_peaks()
+        fu_bytes = FIELD_UPDATE_BYTES_PER_CELL * wl.n_cells
+        fu = {"kernel": "pic_yee_kernel (B half, E, B half fused; writes the plain arrays and the TMA copy)",
+              "ms_per_update": fu_ms, "cells": wl.n_cells, "bytes_per_cell": FIELD_UPDATE_BYTES_PER_CELL,
+              "bound": "hbm", "achieved": fu_bytes / (fu_ms * 1e-3) / 1e9, "peak": peak_f, "unit": "GB/s",
+              "frac": fu_bytes / (fu_ms * 1e-3) / 1e9 / peak_f,
+              "l2": ("working set %.0f MB %s the 126 MB L2" % (fu_bytes / 1e6, "exceeds" if fu_bytes > 126e6 else "fits")),
+              "share_of_self_consistent_step": fu_ms / (fu_ms + ms_max / K)}
     pic.destroy()
 
     e2e = measure_e2e(args, wl, n, K, fields, fresh, barrier, dev, world) if args.e2e_steps > 0 else None
@@ -309,7 +336,7 @@ def run_ours(args):
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": f"inputs larger than L2: {n * 72 / 1e6:.0f} MB of particle state per step vs 126 MB",
                        "tma": args.tma, "deposit": "fixed-point int32 pair" if args.deposit else "float atomics",
-                       "leavers_per_step": stats["leavers_last"]},
+                       "leavers_per_step": stats["leavers_last"], "self_consistent": args.self_consistent},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": traffic, "peak_source": peak_src,
                          "kernel": "pic_step_kernel (resort of the previous step fused into its prologue) "
@@ -324,6 +351,7 @@ def run_ours(args):
                          "ncu": ncu_extra},
             "cpu_baseline": cpu,
             "e2e": e2e,
+            "field_update": fu,
             "gpu_launches": launches, "clocks": clocks,
         }))
     if world > 1:
@@ -344,6 +372,11 @@ def main():
     ap.add_argument("--two-phase", type=int, default=1, help="1: per-cell stencil in registers (two-phase items), 0: gather per particle from the shared tile")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--field-update-reps", type=int, default=20,
+                    help="also time this many launches of the Yee field update alone (0 = skip); not part of the metric")
+    ap.add_argument("--self-consistent", type=int, default=0,
+                    help="1: every timed step ends with the Yee field update (option field_update); the metric's "
+                         "configuration is 0, static fields")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
