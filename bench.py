@@ -302,7 +302,7 @@ def run_ours(args):
               "bound": "hbm", "achieved": fu_bytes / (fu_ms * 1e-3) / 1e9, "peak": peak_f, "unit": "GB/s",
               "frac": fu_bytes / (fu_ms * 1e-3) / 1e9 / peak_f,
               "l2": ("working set %.0f MB %s the 126 MB L2" % (fu_bytes / 1e6, "exceeds" if fu_bytes > 126e6 else "fits")),
-              "share_of_self_consistent_step": fu_ms / (fu_ms + ms_max / K)}
+              "share_of_self_consistent_step": fu_ms / (ms_max / K if args.self_consistent else fu_ms + ms_max / K)}
     pic.destroy()
 
     e2e = measure_e2e(args, wl, n, K, fields, fresh, barrier, dev, world) if args.e2e_steps > 0 else None
