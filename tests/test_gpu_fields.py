@@ -27,11 +27,12 @@ def _vacuum(grid, order):
     return wl, Pic(wl.grid, wl.cell, wl.dt, wl.supercell, wl.shape_order, max_particles=0)
 
 
-@pytest.mark.parametrize("grid", [(16, 16, 8), (40, 24, 20), (64, 16, 12), (8, 8, 4)])
-@pytest.mark.parametrize("order", (2, 3))
-def test_vacuum_update_matches_oracle(grid, order):
-    """No particles (J = 0): grids smaller than one 32x8x8 tile, ragged tiles, several tiles."""
+@pytest.mark.parametrize("grid", [(16, 16, 8), (40, 24, 20), (64, 16, 12), (8, 8, 4), (72, 40, 80)])
+@pytest.mark.parametrize("order,tile", ((2, 8), (3, 8), (2, 4), (3, 16)))
+def test_vacuum_update_matches_oracle(grid, order, tile):
+    """No particles (J = 0): grids smaller than one 32 x tile tile, ragged tiles, several tiles, several z chunks."""
     wl, pic = _vacuum(grid, order)
+    pic.set_option("yee_tile", tile)
     F0 = W.make_fields(wl)
     pic.set_fields(F0.cuda().contiguous())
     F = [f.astype(np.float64) for f in F0.numpy()]
