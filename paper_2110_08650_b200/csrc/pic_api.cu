@@ -26,7 +26,7 @@ struct pic_ctx {
     bool field_update;           // option "field_update": every step ends with a Yee update of E, B (pic_fields.cu)
     float* Fbuf[2];              // the two plain field buffers; d.F == Fbuf[F_cur]
     int F_cur;
-    int yee_tile;                // option "yee_tile": y extent of the Yee kernel's tile (4, 8 or 16)
+    int yee_tile;                // option "yee_tile": y extent of the Yee kernel's tile (8 or 16)
     bool dirty;                  // pool cur holds a stepped state whose sort is still pending
     int force_class;             // option "class_all": -1 = from the counters (default), 0/1/2 = PicDev::class_all as given
     int max_known, min_known;    // largest / smallest non-empty supercell population as of the last synchronisation (0: unknown)
@@ -741,7 +741,7 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
     if (!strcmp(key, "fuse_sort")) { c->fuse_sort = value != 0; return PIC_OK; }
     if (!strcmp(key, "field_update")) { c->field_update = value != 0; return PIC_OK; }
     if (!strcmp(key, "yee_tile")) {
-        if (value != 4 && value != 8 && value != 16) return fail(c, PIC_EINVAL, "pic_set_option: yee_tile must be 4, 8 or 16");
+        if (value != 8 && value != 16) return fail(c, PIC_EINVAL, "pic_set_option: yee_tile must be 8 or 16");
         c->yee_tile = (int)value;
         return PIC_OK;
     }
