@@ -121,6 +121,22 @@ def oracle_sample_rate(wl, n_sample: int, n_steps: int = 1):
     return orc.n * n_steps / dt, dt, orc.n
 
 
+def oracle_field_update_rate(grid=(128, 128, 64), reps=3):
+    """The fp64 numpy oracle of the Yee update (oracle/yee_oracle.py), as it stands, on a bounded grid."""
+    import numpy as np
+    from oracle import yee_oracle as Y
+    rng = np.random.default_rng(0)
+    shp = (grid[2], grid[1], grid[0])
+    F = [rng.normal(size=shp) for _ in range(6)]
+    J = [rng.normal(size=shp) for _ in range(3)]
+    t0 = time.perf_counter()
+    for _ in range(reps):
+        F = Y.yee_update(F, J, 0.5)
+    dt = time.perf_counter() - t0
+    return {"value": reps * grid[0] * grid[1] * grid[2] / dt, "unit": "cell-updates/s", "cores": 1, "kind": "oracle",
+            "sample": f"{reps} updates of a {grid[0]}x{grid[1]}x{grid[2]} grid ({dt:.1f} s), numpy fp64"}
+
+
 def reduce_max_over_ranks(values, device, world: int):
     """MAX over ranks of a list of floats (device time of the slowest rank decides); identity at N=1."""
     import torch
@@ -302,7 +318,10 @@ def run_ours(args):
               "bound": "hbm", "achieved": fu_bytes / (fu_ms * 1e-3) / 1e9, "peak": peak_f, "unit": "GB/s",
               "frac": fu_bytes / (fu_ms * 1e-3) / 1e9 / peak_f,
               "l2": ("working set %.0f MB %s the 126 MB L2" % (fu_bytes / 1e6, "exceeds" if fu_bytes > 126e6 else "fits")),
+              "updates_per_s_cells": wl.n_cells / (fu_ms * 1e-3),
               "share_of_self_consistent_step": fu_ms / (ms_max / K if args.self_consistent else fu_ms + ms_max / K)}
+        if not args.no_cpu_baseline:
+            fu["cpu_baseline"] = oracle_field_update_rate()
     pic.destroy()
 
     e2e = measure_e2e(args, wl, n, K, fields, fresh, barrier, dev, world) if args.e2e_steps > 0 else None

@@ -140,4 +140,6 @@ def test_update_before_set_fields_is_a_state_error():
         pic.update_fields()
     with pytest.raises(PicError):
         pic.get_fields()
+    with pytest.raises(PicError):
+        pic.set_option("yee_tile", 5)
     pic.destroy()
