@@ -168,6 +168,8 @@ int32_t pic_sync(pic_ctx* ctx);
  * supercell in its prologue; 0 = a separate sort kernel before every step; default 1),
  * key "field_update" (1 = every step of pic_step ends with pic_update_fields: the self-consistent loop; default 0),
  * key "yee_tile" (8 or 16, default 8: y extent of the field-update kernel's 32-wide tile; same results),
+ * key "yee_index64" (1 = the field-update kernel indexes with 64 bits, as it does by itself once the padded six-component
+ * array exceeds 2^32 elements; default 0; same results),
  * key "class_all" (-1 = decide from the population counters read at the last synchronisation which kernel
  * variants a step launches — default; 1 = the sparse variant takes every supercell, 2 = the dense variants
  * take every supercell, 0 = classify every supercell by its population and launch all variants),

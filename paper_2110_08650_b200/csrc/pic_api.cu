@@ -26,6 +26,7 @@ struct pic_ctx {
     bool field_update;           // option "field_update": every step ends with a Yee update of E, B (pic_fields.cu)
     float* Fbuf[2];              // the two plain field buffers; d.F == Fbuf[F_cur]
     int F_cur;
+    bool yee_index64;            // option "yee_index64": force the 64-bit-index instantiation (taken anyway beyond 2^32 elements)
     int yee_tile;                // option "yee_tile": y extent of the Yee kernel's tile (8 or 16)
     bool dirty;                  // pool cur holds a stepped state whose sort is still pending
     int force_class;             // option "class_all": -1 = from the counters (default), 0/1/2 = PicDev::class_all as given
@@ -398,6 +399,7 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     c->fuse_sort = true;
     c->field_update = false;
     c->yee_tile = 8;
+    c->yee_index64 = false;
     c->dirty = false;
     c->max_known = c->min_known = 0;
     c->force_class = -1;
@@ -544,7 +546,7 @@ static int ensure_sorted(pic_ctx* c)
 // One Yee update with the last step's J: level n in Fbuf[F_cur] -> level n+1 in the other buffer and in Fpad.
 static cudaError_t enqueue_field_update(pic_ctx* c, cudaStream_t st)
 {
-    cudaError_t e = pic_launch_yee(c->d, c->Fbuf[c->F_cur], c->Fbuf[c->F_cur ^ 1], c->dt, c->cell, c->yee_tile, st, &c->launches);
+    cudaError_t e = pic_launch_yee(c->d, c->Fbuf[c->F_cur], c->Fbuf[c->F_cur ^ 1], c->dt, c->cell, c->yee_tile, c->yee_index64, st, &c->launches);
     if (e != cudaSuccess) return e;
     c->F_cur ^= 1;
     c->d.F = c->Fbuf[c->F_cur];
@@ -740,6 +742,7 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
     }
     if (!strcmp(key, "fuse_sort")) { c->fuse_sort = value != 0; return PIC_OK; }
     if (!strcmp(key, "field_update")) { c->field_update = value != 0; return PIC_OK; }
+    if (!strcmp(key, "yee_index64")) { c->yee_index64 = value != 0; return PIC_OK; }
     if (!strcmp(key, "yee_tile")) {
         if (value != 8 && value != 16) return fail(c, PIC_EINVAL, "pic_set_option: yee_tile must be 8 or 16");
         c->yee_tile = (int)value;

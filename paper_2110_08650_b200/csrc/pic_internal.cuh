@@ -142,4 +142,4 @@ cudaError_t pic_launch_scatter(const PicDev& d, cudaStream_t st, int64_t* launch
 cudaError_t pic_launch_sort(const PicDev& d, cudaStream_t st, int64_t* launches);   // pool cur -> the other
 // pic_fields.cu: one Yee update F_in (level n) -> F_out (level n+1) and the padded copy d.Fpad, with J = d.J
 cudaError_t pic_launch_yee(const PicDev& d, const float* F_in, float* F_out, double dt, const double cell[3], int tile_y,
-                           cudaStream_t st, int64_t* launches);
+                           bool index64, cudaStream_t st, int64_t* launches);

@@ -48,6 +48,54 @@ def test_vacuum_update_matches_oracle(grid, order, tile):
     pic.destroy()
 
 
+def test_index64_variant_matches_the_default_bit_for_bit():
+    """The 64-bit-index instantiation (taken by itself beyond 2^32 elements) on a small grid."""
+    out = []
+    for idx64 in (0, 1):
+        wl, pic = _vacuum((40, 24, 20), 3)
+        pic.set_option("yee_index64", idx64)
+        pic.set_fields(W.make_fields(wl).cuda().contiguous())
+        for _ in range(3):
+            pic.update_fields()
+        out.append(pic.get_fields().cpu())
+        pic.destroy()
+    assert torch.equal(out[0], out[1])
+
+
+@pytest.mark.parametrize("name", ("lwfa", "pqs_large"))
+def test_full_size_grid_sampled_boxes(name):
+    """The grids of configs[2] and configs[4] (67 M cells, the launch configuration bench.py times: 64-plane z chunks),
+    two updates of seeded random fields (no particles: J = 0) against the oracle on sampled boxes: the update of a cell depends on cells within 2 of it per update, so the oracle run on a
+    box cut out of the global arrays (wrapped periodically) is exact 4 cells inside the box."""
+    from paper_2110_08650_b200.binding import Pic
+    wl = W.CONFIGS[name]
+    nx, ny, nz = wl.grid
+    pic = Pic(wl.grid, wl.cell, wl.dt, wl.supercell, wl.shape_order, max_particles=0)
+    g = torch.Generator(device="cuda").manual_seed(5)
+    F0 = (torch.rand((6, nz, ny, nx), device="cuda", generator=g) - 0.5) * 0.1
+    pic.set_fields(F0)
+    n_up, B, M = 2, 24, 4
+    for _ in range(n_up):
+        pic.update_fields()
+    G = pic.get_fields()
+    pic.sync()
+    # boxes at the periodic corner, across the z-chunk boundary at k = 64, and in the interior
+    for lo in ((-12, -12, -12), (100, 500, 52), (nx - 20, 7, nz - 10), (31, ny - 13, 120)):
+        ix = torch.arange(lo[0], lo[0] + B, device="cuda") % nx
+        iy = torch.arange(lo[1], lo[1] + B, device="cuda") % ny
+        iz = torch.arange(lo[2], lo[2] + B, device="cuda") % nz
+        cut = lambda A: A[:, iz][:, :, iy][:, :, :, ix].cpu().numpy().astype(np.float64)
+        F = list(cut(F0))
+        zero = [np.zeros_like(F[0])] * 3
+        for _ in range(n_up):
+            F = Y.yee_update(F, zero, wl.dt, wl.cell)
+        got = cut(G)[:, M:-M, M:-M, M:-M]
+        exp = np.stack(F)[:, M:-M, M:-M, M:-M]
+        err = np.abs(got - exp).max() / 0.05
+        assert err <= n_up * TOL_F, (lo, err)
+    pic.destroy()
+
+
 def test_plane_wave_against_the_closed_form():
     """40 updates of a discrete plane wave (oblique k) against the analytic solution with the numerical
     dispersion relation (derivation: tests/test_oracle_yee.py) — no oracle involved."""
