@@ -140,3 +140,24 @@ def gpu_continuity(wl: W.Workload, pic, q_of_species) -> float:
            + (Jz - np.roll(Jz, 1, 0)) / cell[2])
     drho = (rho1 - rho0) / wl.dt
     return float(np.abs(drho + div).max() / np.abs(drho).max())
+
+
+def energies(fields6, ux, uy, uz, w, cell, mass=1.0):
+    """(electric, magnetic, kinetic) energy with c = eps0 = mu0 = 1: 1/2 sum F^2 dV and sum w m (gamma - 1).
+    E, B at the integer time level, u at the half level before it (the state both sides hold)."""
+    F = [np.asarray(f, dtype=np.float64) for f in fields6]
+    V = cell[0] * cell[1] * cell[2]
+    ef = 0.5 * V * sum(float((f * f).sum()) for f in F[:3])
+    bf = 0.5 * V * sum(float((f * f).sum()) for f in F[3:6])
+    u2 = np.asarray(ux, np.float64) ** 2 + np.asarray(uy, np.float64) ** 2 + np.asarray(uz, np.float64) ** 2
+    ek = float((np.asarray(w, np.float64) * mass * (np.sqrt(1.0 + u2) - 1.0)).sum())
+    return ef, bf, ek
+
+
+def warm_dilute_plasma(order, grid=(16, 16, 16)):
+    """Self-consistent test case: lambda_Debye = u_th/omega_p = 0.1/0.1 = one cell, field and kinetic energy of the
+    same order, so the two reservoirs visibly exchange energy."""
+    wl = W.CONFIGS["thermal_128"].scaled(grid, shape_order=order, ppc=8, u_th=0.1)
+    parts, fields = W.make_particles(wl), W.make_fields(wl)
+    parts.w.mul_(0.00125)
+    return wl, parts, fields

@@ -181,6 +181,28 @@ def test_gauss_law_is_kept_on_the_gpu(order):
     pic.destroy()
 
 
+def test_energies_after_forty_self_consistent_steps():
+    """Free-running 40 steps of the warm dilute plasma (tests/pic_parity.py): electric, magnetic and kinetic energy
+    of the GPU state against the oracle's, each to 1e-5 relative (integrated quantities: the per-particle and
+    per-cell rounding differences average out), and the total within 1 % of its initial value."""
+    wl, parts, fields = PP.warm_dilute_plasma(2)
+    orc = PP.oracle_for(wl, parts, fields)
+    pic = PP.gpu_for(wl, parts, fields, field_update=1)
+    e_start = PP.energies(fields.numpy(), parts.ux.numpy(), parts.uy.numpy(), parts.uz.numpy(), parts.w.numpy(), wl.cell)
+    assert orc.step(40, update_fields=True) == 0
+    pic.step(40)
+    pic.sync()
+    G = PP.gpu_particles_by_id(pic)
+    eg = PP.energies(pic.get_fields().cpu().numpy(), G["ux"], G["uy"], G["uz"], G["w"], wl.cell)
+    O = orc.particles()
+    eo = PP.energies(orc.fields, O["ux"], O["uy"], O["uz"], O["w"], wl.cell)
+    print(f"\n[energies after 40 steps] gpu {eg}  oracle {eo}  start {e_start}")
+    for a, b in zip(eg, eo):
+        assert abs(a - b) <= 1e-5 * abs(b)
+    assert abs(sum(eg) / sum(e_start) - 1) < 1e-2
+    pic.destroy()
+
+
 def test_update_before_set_fields_is_a_state_error():
     from paper_2110_08650_b200.binding import Pic, PicError
     pic = Pic((16, 16, 8), shape_order=1, max_particles=0)
