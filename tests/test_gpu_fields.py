@@ -203,6 +203,56 @@ def test_energies_after_forty_self_consistent_steps():
     pic.destroy()
 
 
+def test_full_size_self_consistent_loop_keeps_gauss_law():
+    """configs[1] at full size (128^3 cells, 33.5 M particles, TSC; weights scaled to omega_p*dt = 0.2 so that the closed
+    loop is stable), three steps with option field_update in the launch configuration bench.py --self-consistent times.
+    Properties that hold at any size: no device fault, ids a permutation, membership consistent; and on a sampled box
+    div E - rho (rho in fp64 from the GPU's own positions, all particles within reach of the box) stays what it was."""
+    from paper_2110_08650_b200.binding import Pic
+    wl = W.CONFIGS["thermal_128"]
+    n = W.n_particles(wl)
+    dev = "cuda:0"
+    pic = Pic(wl.grid, wl.cell, wl.dt, wl.supercell, wl.shape_order, max_particles=n, device=dev)
+    keys = ("x", "y", "z", "ux", "uy", "uz", "w", "species")
+    for chunk in W.particle_chunks(wl, device=dev, max_chunk=1 << 23):
+        chunk.w.mul_(0.01)
+        pic.load_particles(*(getattr(chunk, k) for k in keys))
+        pic.sync()
+    del chunk
+    pic.set_fields(W.make_fields(wl, device=dev))
+    pic.set_option("field_update", 1)
+    lo, B, M = (50, 60, 28), 24, 4          # box spans supercell faces and the z-chunk boundary of the Yee kernel at k = 32
+    prm = oracle.OracleParams.make((B, B, B), wl.cell, wl.dt, wl.supercell, wl.shape_order)
+
+    def gauss():
+        P = pic.get_particles()
+        inb = torch.ones(P["x"].numel(), dtype=torch.bool, device=dev)
+        for a, k in enumerate("xyz"):
+            inb &= (P[k] >= lo[a]) & (P[k] < lo[a] + B)
+        q = {k: P[k][inb].cpu().numpy() for k in ("x", "y", "z", "w")}
+        rho = oracle.rho(prm, q["x"] - lo[0], q["y"] - lo[1], q["z"] - lo[2], -q["w"].astype(np.float64))
+        E = pic.get_fields()[:3, lo[2] - 1:lo[2] + B, lo[1] - 1:lo[1] + B, lo[0] - 1:lo[0] + B].cpu().numpy().astype(np.float64)
+        div = ((E[0][1:, 1:, 1:] - E[0][1:, 1:, :-1]) + (E[1][1:, 1:, 1:] - E[1][1:, :-1, 1:])
+               + (E[2][1:, 1:, 1:] - E[2][:-1, 1:, 1:]))
+        sl = (slice(M, -M),) * 3
+        return (div - rho)[sl], float(np.abs(rho[sl]).max())
+
+    g0, rmax = gauss()
+    n_steps = 3
+    pic.step(n_steps)
+    pic.sync()
+    st = pic.get_stats()
+    assert st["error"] == 0 and st["particles"] == n and st["steps"] == n_steps
+    g1, _ = gauss()
+    drift = float(np.abs(g1 - g0).max()) / rmax
+    print(f"\n[full-size loop] drift of (div E - rho) / max|rho| in the box after {n_steps} steps = {drift:.3e}")
+    assert drift <= n_steps * PP.TOL_CONT
+    ids = pic.get_particles()["id"].to(torch.int64) & 0xFFFFFFFF
+    assert torch.equal(torch.sort(ids).values, torch.arange(n, device=dev))
+    assert PP.gpu_membership_consistent(wl, pic)
+    pic.destroy()
+
+
 def test_update_before_set_fields_is_a_state_error():
     from paper_2110_08650_b200.binding import Pic, PicError
     pic = Pic((16, 16, 8), shape_order=1, max_particles=0)
