@@ -124,3 +124,58 @@ def test_generators_other_layouts():
     assert float(fl[0].abs().max()) > 1.0 and float(fl[1].abs().max()) == 0.0
     fm = W.make_fields(W.CONFIGS["thermal_128"].scaled((16, 16, 16)))
     assert float(fm.abs().max()) <= 0.01 + 1e-7 and float(fm.abs().max()) > 1e-3
+
+
+def test_step_uses_charge_over_mass_per_species():
+    """Pins the per-species q/m inside Oracle.step: two species (q, m) = (-1, 1) and
+    (2, 3).  (a) B = 0, uniform E: u_new - u = (q/m) E dt exactly (SURVEY.md §8(c) step 4 pin (iii));
+    (b) E = 0, uniform B: |u| is kept and u turns by exactly 2 atan(|q/m| |B| dt / (2 gamma)) in the sense
+    of -q/m (pin (ii)); (c) the deposited current still carries the CHARGE q (not q/m): total current
+    sum J_a V = sum_p q w dX_a dx_a / dt (step 6 pin (iii)).  A step that used q, m or q*m for the push, or
+    q/m for the deposit, fails one of them."""
+    grid, dt = (8, 8, 8), 0.5
+    q, m = np.array([-1.0, 2.0]), np.array([1.0, 3.0])
+    rng = np.random.default_rng(5)
+    n = 64
+    X = rng.uniform(0, 8, (3, n))
+    u0 = rng.normal(0, 0.3, (3, n))
+    w = rng.uniform(0.5, 1.5, n)
+    sp = (np.arange(n) % 2).astype(np.int32)
+    qm = (q / m)[sp]
+    for order in (1, 2, 3):
+        # (a) impulse
+        orc = oracle.Oracle(grid, dt=dt, order=order)
+        orc.set_species(q, m)
+        orc.load_particles(*X, *u0, w, species=sp)
+        F = np.zeros((6,) + grid[::-1])
+        E = np.array([0.02, -0.01, 0.03])
+        for a in range(3):
+            F[a] = E[a]
+        orc.set_fields(F)
+        assert orc.step(1) == 0
+        P = orc.particles()
+        un = np.stack([P["ux"], P["uy"], P["uz"]])
+        np.testing.assert_allclose(un - u0, qm[None, :] * E[:, None] * dt, rtol=0, atol=1e-15)
+        # (c) total current carries q (times w), not q/m
+        g = np.sqrt(1 + (un ** 2).sum(0))
+        dX = un / g * dt
+        for a in range(3):
+            np.testing.assert_allclose(orc.J[a].sum(), ((q[sp] * w) * dX[a]).sum() / dt, rtol=1e-12)
+        # (b) rotation
+        orc = oracle.Oracle(grid, dt=dt, order=order)
+        orc.set_species(q, m)
+        orc.load_particles(*X, *u0, w, species=sp)
+        F = np.zeros((6,) + grid[::-1])
+        Bz = 0.4
+        F[5] = Bz
+        orc.set_fields(F)
+        assert orc.step(1) == 0
+        P = orc.particles()
+        un = np.stack([P["ux"], P["uy"], P["uz"]])
+        np.testing.assert_allclose((un ** 2).sum(0), (u0 ** 2).sum(0), rtol=1e-14)
+        np.testing.assert_allclose(un[2], u0[2], rtol=0, atol=1e-16)
+        gam = np.sqrt(1 + (u0 ** 2).sum(0))
+        ang = np.arctan2(un[1], un[0]) - np.arctan2(u0[1], u0[0])
+        ang = (ang + np.pi) % (2 * np.pi) - np.pi
+        # du/dt = (q/m) u x B / gamma: for B along +z the perpendicular momentum turns by -(q/m)|B|dt/gamma
+        np.testing.assert_allclose(ang, -np.sign(qm) * 2 * np.arctan(np.abs(qm) * Bz * dt / (2 * gam)), rtol=0, atol=1e-13)
