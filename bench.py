@@ -264,6 +264,7 @@ def run_ours(args):
         pic.set_option("deposit", args.deposit)
         pic.set_option("segment", args.segment)
         pic.set_option("two_phase", args.two_phase)
+        pic.set_option("cell_kernel", args.cell_kernel)
         pic.set_option("field_update", args.self_consistent)
         return pic
 
@@ -389,6 +390,7 @@ def main():
     ap.add_argument("--deposit", type=int, default=1, help="1 fixed-point integer atomics, 0 float CAS atomics")
     ap.add_argument("--segment", type=int, default=3, help="work-item length in quarters of the mean cell population")
     ap.add_argument("--two-phase", type=int, default=1, help="1: per-cell stencil in registers (two-phase items), 0: gather per particle from the shared tile")
+    ap.add_argument("--cell-kernel", type=int, default=0, help="1: dense supercells go to pic_cell_kernel (third generation), 0: round-1 kernels")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--field-update-reps", type=int, default=20,

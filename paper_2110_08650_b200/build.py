@@ -14,8 +14,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpic_b200.so")
-SOURCES = ("pic_api.cu", "pic_step.cu", "pic_fields.cu")
-HEADERS = ("pic_internal.cuh", "pic_device.cuh", os.path.join("..", "..", "include", "pic_b200.h"))
+SOURCES = ("pic_api.cu", "pic_step.cu", "pic_cell.cu", "pic_fields.cu")
+HEADERS = ("pic_internal.cuh", "pic_device.cuh", "pic_step_common.cuh", os.path.join("..", "..", "include", "pic_b200.h"))
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC", "-cudart", "static",
@@ -52,19 +52,28 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
         return LIB
     hdr_t = max(os.path.getmtime(os.path.join(CSRC, h)) for h in HEADERS)
     hdr_t = max(hdr_t, os.path.getmtime(os.path.abspath(__file__)))
-    objs = []
+    objs, jobs = [], []
     for s in SOURCES:
         src = os.path.join(CSRC, s)
         obj = os.path.join(CSRC, s[:-3] + ".o")
         objs.append(obj)
         if force or not os.path.exists(obj) or os.path.getmtime(obj) < max(hdr_t, os.path.getmtime(src)):
-            tmp = obj + f".tmp{os.getpid()}"
-            try:
-                _run([_nvcc(), *(["-Xptxas", "-v"] if verbose else []), *NVCC_FLAGS, "-c", "-o", tmp, src], verbose)
-                os.replace(tmp, obj)
-            finally:
-                if os.path.exists(tmp):
-                    os.remove(tmp)
+            jobs.append((src, obj))
+
+    def compile_one(job):
+        src, obj = job
+        tmp = obj + f".tmp{os.getpid()}"
+        try:
+            _run([_nvcc(), *(["-Xptxas", "-v"] if verbose else []), *NVCC_FLAGS, "-c", "-o", tmp, src], verbose)
+            os.replace(tmp, obj)
+        finally:
+            if os.path.exists(tmp):
+                os.remove(tmp)
+
+    if jobs:      # one nvcc per translation unit, side by side
+        from concurrent.futures import ThreadPoolExecutor
+        with ThreadPoolExecutor(max_workers=len(jobs)) as ex:
+            list(ex.map(compile_one, jobs))
     tmp = LIB + f".tmp{os.getpid()}"
     try:
         _run([_nvcc(), *NVCC_FLAGS, "-shared", "-o", tmp, *objs], verbose)

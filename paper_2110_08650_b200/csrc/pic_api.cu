@@ -22,6 +22,7 @@ struct pic_ctx {
     cudaStream_t stream;
     bool have_fields;
     bool use_tma, use_graph, fixed_point;
+    bool cell_kernel;            // option "cell_kernel": dense supercells go to pic_cell_kernel (default on)
     bool fuse_sort;              // option "fuse_sort": the step kernel sorts its supercell first (default on)
     bool field_update;           // option "field_update": every step ends with a Yee update of E, B (pic_fields.cu)
     float* Fbuf[2];              // the two plain field buffers; d.F == Fbuf[F_cur]
@@ -397,6 +398,7 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     c->use_tma = true;
     c->use_graph = false;
     c->fuse_sort = true;
+    c->cell_kernel = false;      // measured slower than the round-1 two-phase kernel so far (profiles/README.md)
     c->field_update = false;
     c->yee_tile = 8;
     c->yee_index64 = false;
@@ -593,7 +595,7 @@ static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
             ds.sort_filter = d.class_all == 1 ? 0 : 1;
             if (e == cudaSuccess) e = pic_launch_sort(ds, st, &c->launches);
         }
-        if (e == cudaSuccess) e = pic_launch_step(d, c->order, c->use_tma && c->tmap_ok, c->fixed_point, c->tmap, st, &c->launches);
+        if (e == cudaSuccess) e = pic_launch_step(d, c->order, c->use_tma && c->tmap_ok, c->fixed_point, c->tmap, st, &c->launches, c->cell_kernel);
         d.fused = 0;
         if (e == cudaSuccess && c->timing) {
             e = cudaEventRecord(ev1, st);
@@ -741,6 +743,7 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
         return PIC_OK;
     }
     if (!strcmp(key, "fuse_sort")) { c->fuse_sort = value != 0; return PIC_OK; }
+    if (!strcmp(key, "cell_kernel")) { c->cell_kernel = value != 0; return PIC_OK; }
     if (!strcmp(key, "field_update")) { c->field_update = value != 0; return PIC_OK; }
     if (!strcmp(key, "yee_index64")) { c->yee_index64 = value != 0; return PIC_OK; }
     if (!strcmp(key, "yee_tile")) {

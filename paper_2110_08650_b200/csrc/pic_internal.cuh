@@ -123,6 +123,7 @@ __host__ __device__ inline int pic_segment_target(int supercell_count, int seg_n
 {
     int t = (seg_num * supercell_count + 1023) / 1024;     // seg_num/4 of the mean cell population
     if (t < 4) t = 4;
+    if (t > 256) t = 256;      // PIC_FLUSH_MAX: the fixed-point split of a register sum is exact for <= 256 contributions
     if (lmax > 0 && supercell_count <= 768 * lmax) t = lmax;    // two-phase: items as long as the staging allows
     return t;
 }
@@ -134,7 +135,9 @@ __host__ __device__ inline uint32_t pic_pack_bits(int local_cell, int species)
 
 // launchers implemented in pic_step.cu
 cudaError_t pic_launch_step(const PicDev& d, int order, bool use_tma, bool fixed_point, const void* tmap,
-                            cudaStream_t st, int64_t* launches);
+                            cudaStream_t st, int64_t* launches, bool cell_kernel);
+// pic_cell.cu: the dense whole-cell kernel (fixed point), launched over all supercells; sparse ones exit
+cudaError_t pic_launch_cell(const PicDev& d, int order, bool use_tma, const void* tmap, cudaStream_t st, int64_t* launches);
 cudaError_t pic_launch_overflow(const PicDev& d, int order, bool fixed_point, cudaStream_t st, int64_t* launches);
 cudaError_t pic_launch_convert(const PicDev& d, cudaStream_t st, int64_t* launches);
 cudaError_t pic_launch_prepare(const PicDev& d, cudaStream_t st, int64_t* launches);
