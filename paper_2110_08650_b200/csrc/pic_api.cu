@@ -22,7 +22,7 @@ struct pic_ctx {
     cudaStream_t stream;
     bool have_fields;
     bool use_tma, use_graph, fixed_point;
-    bool cell_kernel;            // option "cell_kernel": dense supercells go to pic_cell_kernel (default on)
+    int cell_kernel;             // option "cell_kernel": dense supercells go to 0 the round-1 kernels, 1 pic_cell_kernel, 2 the persistent pic_pcell_kernel
     bool fuse_sort;              // option "fuse_sort": the step kernel sorts its supercell first (default on)
     bool field_update;           // option "field_update": every step ends with a Yee update of E, B (pic_fields.cu)
     float* Fbuf[2];              // the two plain field buffers; d.F == Fbuf[F_cur]
@@ -398,7 +398,7 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     c->use_tma = true;
     c->use_graph = false;
     c->fuse_sort = true;
-    c->cell_kernel = false;      // measured slower than the round-1 two-phase kernel so far (profiles/README.md)
+    c->cell_kernel = 0;
     c->field_update = false;
     c->yee_tile = 8;
     c->yee_index64 = false;
@@ -571,6 +571,7 @@ static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
                                        : cudaMemsetAsync(d.J, 0, 3 * ncell * sizeof(float), st);
         if (e == cudaSuccess) e = cudaMemsetAsync(d.ctr + CTR_EXCH, 0, sizeof(int), st);
         if (e == cudaSuccess) e = cudaMemsetAsync(d.ctr + CTR_OVF, 0, sizeof(int), st);
+        if (e == cudaSuccess && c->cell_kernel == 2) e = cudaMemsetAsync(d.ctr + CTR_WORK, 0, sizeof(int), st);
         cudaEvent_t ev0 = nullptr, ev1 = nullptr;
         if (e == cudaSuccess && c->timing) {
             e = cudaEventCreate(&ev0);
@@ -743,7 +744,11 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
         return PIC_OK;
     }
     if (!strcmp(key, "fuse_sort")) { c->fuse_sort = value != 0; return PIC_OK; }
-    if (!strcmp(key, "cell_kernel")) { c->cell_kernel = value != 0; return PIC_OK; }
+    if (!strcmp(key, "cell_kernel")) {
+        if (value < 0 || value > 2) return fail(c, PIC_EINVAL, "pic_set_option: cell_kernel must be 0, 1 or 2");
+        c->cell_kernel = (int)value;
+        return PIC_OK;
+    }
     if (!strcmp(key, "field_update")) { c->field_update = value != 0; return PIC_OK; }
     if (!strcmp(key, "yee_index64")) { c->yee_index64 = value != 0; return PIC_OK; }
     if (!strcmp(key, "yee_tile")) {

@@ -35,6 +35,7 @@ enum {
     CTR_OVF = 7,
     CTR_FREE_TOP = 8,     // entries on the stack of returned frames (may dip below 0 while prepare pops)          // entries in the overflow queue of out-of-window particles (this step)
        // bits of max |weight| loaded so far (non-negative floats order like ints)
+    CTR_WORK = 10,        // next supercell of the persistent step kernel (zeroed before every launch)
     CTR_NEGMIN = 9,       // max over non-empty supercells of (2^30 - population) seen by pic_prepare_kernel, i.e. 2^30 - min
     CTR_N = 16
 };
@@ -135,9 +136,10 @@ __host__ __device__ inline uint32_t pic_pack_bits(int local_cell, int species)
 
 // launchers implemented in pic_step.cu
 cudaError_t pic_launch_step(const PicDev& d, int order, bool use_tma, bool fixed_point, const void* tmap,
-                            cudaStream_t st, int64_t* launches, bool cell_kernel);
+                            cudaStream_t st, int64_t* launches, int cell_kernel);
 // pic_cell.cu: the dense whole-cell kernel (fixed point), launched over all supercells; sparse ones exit
-cudaError_t pic_launch_cell(const PicDev& d, int order, bool use_tma, const void* tmap, cudaStream_t st, int64_t* launches);
+cudaError_t pic_launch_cell(const PicDev& d, int order, bool use_tma, const void* tmap, cudaStream_t st, int64_t* launches,
+                            bool persistent);
 cudaError_t pic_launch_overflow(const PicDev& d, int order, bool fixed_point, cudaStream_t st, int64_t* launches);
 cudaError_t pic_launch_convert(const PicDev& d, cudaStream_t st, int64_t* launches);
 cudaError_t pic_launch_prepare(const PicDev& d, cudaStream_t st, int64_t* launches);

@@ -828,11 +828,11 @@ static cudaError_t launch_step_one(const PicDev& d, const CUtensorMap& map, cuda
 }
 
 template <int O, bool TMA, bool FIX>
-static cudaError_t launch_step_variant(const PicDev& d, const CUtensorMap& map, cudaStream_t st, int64_t* launches, bool cell)
+static cudaError_t launch_step_variant(const PicDev& d, const CUtensorMap& map, cudaStream_t st, int64_t* launches, int cell)
 {
     cudaError_t e = cudaSuccess;
     if (d.class_all != 1 && cell) {     // dense supercells: the whole-cell kernel of pic_cell.cu (fixed point only)
-        e = pic_launch_cell(d, O, TMA, &map, st, launches);
+        e = pic_launch_cell(d, O, TMA, &map, st, launches, cell == 2);
     } else if (d.class_all != 1) {      // dense variants (none when the host knows every supercell to be sparse)
         if (d.two_phase) {
             e = launch_step_one<O, TMA, FIX, PIC_MODE_TWO>(d, map, st);
@@ -851,9 +851,9 @@ static cudaError_t launch_step_variant(const PicDev& d, const CUtensorMap& map, 
 }
 
 cudaError_t pic_launch_step(const PicDev& d, int order, bool use_tma, bool fixed_point, const void* tmap,
-                            cudaStream_t st, int64_t* launches, bool cell_kernel)
+                            cudaStream_t st, int64_t* launches, int cell_kernel)
 {
-    const bool cell = cell_kernel && fixed_point;
+    const int cell = fixed_point ? cell_kernel : 0;
     CUtensorMap map;
     if (use_tma) memcpy(&map, tmap, sizeof map); else memset(&map, 0, sizeof map);
     cudaError_t e;

@@ -265,9 +265,17 @@ __device__ __forceinline__ void finish_particle(const PicDev& d, float4* rec, si
     }
 }
 
+// Barrier over the NT threads that run a block-level routine: the whole CTA (BAR == 0, __syncthreads) or one warp
+// group of a warp-specialized kernel (named barrier BAR > 0; the other warps of the CTA do not take part).
+template <int BAR, int NT> __device__ __forceinline__ void group_sync()
+{
+    if constexpr (BAR == 0) __syncthreads();
+    else asm volatile("bar.sync %0, %1;" ::"n"(BAR), "n"(NT) : "memory");
+}
+
 // ------------------------------------------------------------------ sort fused into the step kernel's prologue
 // Exclusive scan over 256 counts held NT-strided in registers (entry tid*PER + k); two block barriers.
-template <int NT>
+template <int NT, int BAR = 0>
 __device__ __forceinline__ void block_excl_scan256(int (&v)[256 / NT], int& total, int* s_w, int tid)
 {
     constexpr int PER = 256 / NT, NW = NT / 32;
@@ -281,9 +289,9 @@ __device__ __forceinline__ void block_excl_scan256(int (&v)[256 / NT], int& tota
         const int t = __shfl_up_sync(0xffffffffu, inc, o);
         if (lane >= o) inc += t;
     }
-    __syncthreads();               // s_w may still be read from an earlier scan
+    group_sync<BAR, NT>();               // s_w may still be read from an earlier scan
     if (lane == 31) s_w[warp] = inc;
-    __syncthreads();
+    group_sync<BAR, NT>();
     int wb = 0;
     total = 0;
 #pragma unroll
@@ -306,8 +314,13 @@ __device__ __forceinline__ void block_excl_scan256(int (&v)[256 / NT], int& tota
 // Leaves the cell ranges in s_off[0..256] (shared), publishes the new count, clears the global histogram,
 // returns frames the supercell no longer needs.  s_cur: 256 ints of scratch; s_w: 16 ints of scratch.
 #define PIC_SORT_TBL 1024
-template <int NT>
-__device__ __forceinline__ int fused_sort(const PicDev& d, int s, int tid, int* s_off, int* s_cur, int* s_w, int* s_tbl_scr)
+// STAGE_R > 0: the records are not held in registers but requested with cp.async into `scratch` (STAGE_R records per
+// thread and round, 36 bytes each, every thread its own entries): as many loads in flight with a handful of
+// registers — for the producer warps of the persistent kernel, which run on 56 registers (spilled batch registers
+// serialise the loads: the spill store waits for the load).
+template <int NT, int BAR = 0, int U = 4, int STAGE_R = 0>
+__device__ __forceinline__ int fused_sort(const PicDev& d, int s, int tid, int* s_off, int* s_cur, int* s_w, int* s_tbl_scr,
+                                          unsigned char* scratch = nullptr)
 {
     constexpr int PER = 256 / NT;
     const int n_scan = d.sc_tail[s];
@@ -318,7 +331,7 @@ __device__ __forceinline__ int fused_sort(const PicDev& d, int s, int tid, int* 
         d.cell_hist_prev[(size_t)s * 256 + tid * PER + k] = 0;
     }
     int total;
-    block_excl_scan256<NT>(v, total, s_w, tid);
+    block_excl_scan256<NT, BAR>(v, total, s_w, tid);
 #pragma unroll
     for (int k = 0; k < PER; ++k) {
         s_off[tid * PER + k] = v[k];
@@ -328,7 +341,7 @@ __device__ __forceinline__ int fused_sort(const PicDev& d, int s, int tid, int* 
         s_off[256] = total;
         d.sc_count[s] = total;
     }
-    __syncthreads();
+    group_sync<BAR, NT>();
     if (total > n_scan || total != d.sc_next[s]) {      // histogram and records disagree: never write out of bounds
         if (tid == 0) atomicOr(d.ctr + CTR_ERROR, PIC_DEV_SORT_MISMATCH);
         return -1;
@@ -338,15 +351,50 @@ __device__ __forceinline__ int fused_sort(const PicDev& d, int s, int tid, int* 
     const int* tbl = d.tbl_pool + d.tbl_off[s];
     if (have_frames <= PIC_SORT_TBL) {
         for (int t = tid; t < have_frames; t += NT) s_tbl_scr[t] = tbl[t];
-        __syncthreads();
+        group_sync<BAR, NT>();
         tbl = s_tbl_scr;
     }
     const float4* src = d.rec[d.cur ^ 1];
     float4* dst = d.rec[d.cur];
     const uint32_t* sid = d.pid[d.cur ^ 1];
     uint32_t* did = d.pid[d.cur];
+    if constexpr (STAGE_R > 0) {
+        float4* sP = reinterpret_cast<float4*>(scratch);
+        float4* sM = sP + STAGE_R * NT;
+        uint32_t* sI = reinterpret_cast<uint32_t*>(sM + STAGE_R * NT);
+        for (int base = 0; base < n_scan; base += STAGE_R * NT) {
+#pragma unroll
+            for (int u = 0; u < STAGE_R; ++u) {
+                const int slot = base + u * NT + tid;
+                if (slot < n_scan) {
+                    const size_t i = (size_t)tbl[slot >> 8] * PIC_FRAME + (slot & (PIC_FRAME - 1));
+                    cp_async16(sP + u * NT + tid, src + 2 * i);
+                    cp_async16(sM + u * NT + tid, src + 2 * i + 1);
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((uint32_t)__cvta_generic_to_shared(sI + u * NT + tid)),
+                                 "l"(sid + i) : "memory");
+                }
+            }
+            cp_async_wait_all();
+#pragma unroll
+            for (int u = 0; u < STAGE_R; ++u) {
+                const int slot = base + u * NT + tid;
+                if (slot >= n_scan) continue;
+                const float4 M = sM[u * NT + tid];
+                const uint32_t bits = __float_as_uint(M.w);
+                if (bits & PIC_LEFT_FLAG) continue;
+                const int r = atomicAdd(&s_cur[bits & 0xff], 1);
+                if (r >= total) {
+                    atomicOr(d.ctr + CTR_ERROR, PIC_DEV_SORT_MISMATCH);
+                    continue;
+                }
+                const size_t o = (size_t)tbl[r >> 8] * PIC_FRAME + (r & (PIC_FRAME - 1));
+                dst[2 * o] = sP[u * NT + tid];
+                dst[2 * o + 1] = M;
+                did[o] = sI[u * NT + tid];
+            }
+        }
+    } else {
     // U slots per thread and batch; the next batch is loaded while the current one is ranked and stored
-    constexpr int U = 4;
     struct Batch {
         float4 P[U], M[U];
         uint32_t id[U];
@@ -390,7 +438,8 @@ __device__ __forceinline__ int fused_sort(const PicDev& d, int s, int tid, int* 
         load(qa, base + 2 * U * NT);
         place(qb);
     }
-    __syncthreads();                   // the sorted records are visible to the whole CTA
+    }
+    group_sync<BAR, NT>();                   // the sorted records are visible to the whole CTA
     if (tid == 0) {
         const int keep = (total + PIC_FRAME - 1) / PIC_FRAME + 1, have = d.sc_nframes[s];
         if (have > keep) {

@@ -52,6 +52,19 @@ def test_one_step(name, tma):
     pic.destroy()
 
 
+@pytest.mark.parametrize("name", list(CASES))
+@pytest.mark.parametrize("kernel", (0, 1, 2))
+def test_dense_kernel_generations(name, kernel):
+    """Option cell_kernel: 0 the round-1 dense kernels (work items of <= LMAX particles), 1 pic_cell_kernel (one CTA
+    per supercell, one thread per cell), 2 pic_pcell_kernel (persistent CTAs, producer warps sort and stage the
+    next supercell beside the consumer warps).  Each is held to the oracle for three free-running steps (the second
+    and third start from a fused sort of the stepped state)."""
+    rep, pic, wl = _run(name, 3, cell_kernel=kernel)
+    assert rep.max_dx <= 3 * PP.TOL_X and rep.max_du_rel <= 3 * PP.TOL_U and rep.j_err_rel <= PP.TOL_J10
+    assert rep.n_member_mismatch == 0 and rep.counts_equal_outside_band
+    pic.destroy()
+
+
 @pytest.mark.parametrize("name", ["cfg1_tiny_cic", "cfg2_thermal_tsc_32", "cfg5_pqs_32x32x16"])
 def test_float_atomic_deposit_variant(name):
     """Option deposit=0 (float atomics on the shared J tile) computes the same step."""
