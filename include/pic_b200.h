@@ -60,6 +60,7 @@ extern "C" {
 #define PIC_DEV_TMA_TIMEOUT           16
 #define PIC_DEV_OVERFLOW_QUEUE_FULL   32   /* out-of-window particles exceeded the global overflow queue */
 #define PIC_DEV_SORT_MISMATCH         64   /* internal: cell histogram and records disagree */
+#define PIC_DEV_BAD_SPECIES          128   /* a loaded particle names a species id outside the table of pic_set_species */
 
 typedef struct pic_ctx pic_ctx;   /* opaque, host-side */
 
@@ -82,7 +83,10 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
                    void* workspace, uint64_t workspace_bytes, void* stream);
 
 /* Species table (reading S15): charge q[s] and mass m[s], host pointers, n <=
- * PIC_MAX_SPECIES.  Default for every species id: q = -1, m = 1. */
+ * PIC_MAX_SPECIES.  Until the first call every species id in [0, PIC_MAX_SPECIES) has q = -1, m = 1; after a call
+ * with n > 0 the table has n entries: a particle loaded with a species id >= n raises the sticky device fault
+ * PIC_DEV_BAD_SPECIES, and the fixed-point scale of the current follows max|q| over these n entries
+ * (charges of any magnitude, e.g. 1.6e-19, keep the full resolution). */
 int32_t pic_set_species(pic_ctx* ctx, int32_t n, const double* q, const double* m);
 
 /* Append n particles ("pic_load_particles(SoA x/u/weight/species)").  x,y,z: float64
@@ -166,7 +170,17 @@ int32_t pic_sync(pic_ctx* ctx);
  * from the shared tile; default 1),
  * key "fuse_sort" (1 = a step leaves the supercells unsorted and the next step's kernel sorts each dense
  * supercell in its prologue; 0 = a separate sort kernel before every step; default 1),
- * key "field_update" (1 = every step of pic_step ends with pic_update_fields: the self-consistent loop; default 0),
+ * key "field_update" (1 = every step of pic_step ends with pic_update_fields: the self-consistent loop; default 0;
+ * PIC_EINVAL, as from pic_update_fields, unless dt*sqrt(1/dx^2 + 1/dy^2 + 1/dz^2) < 1, the CFL limit of the explicit
+ * Yee scheme — the particle step alone only needs c*dt < cell),
+ * key "cell_kernel" (which kernel steps the dense supercells: 0 = the round-1 kernels of pic_step.cu — work items of at
+ * most 11 particles — default, the fastest measured; 1 = pic_cell_kernel, one thread per cell; 2 = pic_pcell_kernel,
+ * persistent CTAs whose producer warps sort and stage the next supercell beside the consumer warps; same results
+ * within fp32 rounding of the per-cell sums; fixed-point deposit only),
+ * keys "limit_frames", "limit_exchange", "limit_tables" (fault injection for tests: lower the number of particle
+ * frames / exchange-buffer entries / frame-table entries below what the workspace was sized for; only before the
+ * first pic_load_particles; the step then raises PIC_DEV_FRAME_POOL_EXHAUSTED / PIC_DEV_EXCHANGE_OVERFLOW /
+ * PIC_DEV_TABLE_POOL_EXHAUSTED instead of writing out of bounds),
  * key "yee_tile" (8 or 16, default 8: y extent of the field-update kernel's 32-wide tile; same results),
  * key "yee_index64" (1 = the field-update kernel indexes with 64 bits, as it does by itself once the padded six-component
  * array exceeds 2^32 elements; default 0; same results),

@@ -18,10 +18,11 @@ struct pic_ctx {
     int order;
     double cell[3], dt;
     double q[PIC_NSPECIES], m[PIC_NSPECIES];
+    int n_species;               // slots set by pic_set_species (PIC_NSPECIES while the defaults q=-1, m=1 stand)
     int64_t max_particles, n_particles, steps, launches;
     cudaStream_t stream;
     bool have_fields;
-    bool use_tma, use_graph, fixed_point;
+    bool use_tma, fixed_point;
     int cell_kernel;             // option "cell_kernel": dense supercells go to 0 the round-1 kernels, 1 pic_cell_kernel, 2 the persistent pic_pcell_kernel
     bool fuse_sort;              // option "fuse_sort": the step kernel sorts its supercell first (default on)
     bool field_update;           // option "field_update": every step ends with a Yee update of E, B (pic_fields.cu)
@@ -37,11 +38,9 @@ struct pic_ctx {
     char* ws;
     uint64_t ws_bytes;
     std::string err;
-    // TMA descriptor + graph cache (pic_tma.cu / pic_api.cu)
+    // TMA descriptor of the padded field copy
     alignas(64) unsigned char tmap[128];
     bool tmap_ok;
-    cudaGraphExec_t graph_exec;
-    int graph_steps;
     // option "timing": CUDA events around every launch of the step kernel
     bool timing;
     std::vector<cudaEvent_t> events;
@@ -177,6 +176,7 @@ __global__ void pic_load_count_kernel(const PicDev d, const LoadArgs a)
         atomicAdd(d.sc_incoming + s, 1);
         atomicAdd(d.cell_hist + (size_t)s * 256 + lc, 1);
         wmax = max(wmax, __float_as_int(fabsf(a.w[i])));
+        if (a.species && (a.species[i] < 0 || a.species[i] >= d.n_species)) atomicOr(d.ctr + CTR_ERROR, PIC_DEV_BAD_SPECIES);
     }
     // one atomic per warp, and only if it raises the maximum (a per-particle atomicMax on one address
     // serialises in L2: 0.8 ms per 8 M particles)
@@ -298,9 +298,20 @@ void refresh_species(pic_ctx* c)
         c->d.h[s] = (float)((c->q[s] / c->m[s]) * c->dt * 0.5);
         c->d.q[s] = (float)c->q[s];
     }
+    // the fixed-point scale of J follows max|q| over the slots in use only: the default q = -1 of slots the caller
+    // never set must not pin it when the table holds physical charges
     double qmax = 0.0;
-    for (int s = 0; s < PIC_NSPECIES; ++s) qmax = fmax(qmax, fabs(c->q[s]));
+    for (int s = 0; s < c->n_species; ++s) qmax = fmax(qmax, fabs(c->q[s]));
     c->d.qmax = (float)qmax;
+    c->d.n_species = c->n_species;
+}
+
+// explicit Yee scheme: stable for c*dt*sqrt(1/dx^2 + 1/dy^2 + 1/dz^2) < 1 (the particle step alone only needs c*dt < cell)
+bool yee_stable(const pic_ctx* c)
+{
+    double s = 0.0;
+    for (int a = 0; a < 3; ++a) s += 1.0 / (c->cell[a] * c->cell[a]);
+    return c->dt * sqrt(s) < 1.0;
 }
 
 int check_device(pic_ctx* c)
@@ -314,8 +325,8 @@ int check_device(pic_ctx* c)
     c->max_known = ctr[CTR_MAX_COUNT];
     c->min_known = ctr[CTR_NEGMIN] ? (1 << 30) - ctr[CTR_NEGMIN] : 0;
     if (err) {
-        char buf[160];
-        snprintf(buf, sizeof buf, "device fault word 0x%x (1 frame pool, 2 exchange buffer, 4 table pool, 8 moved >= 1 cell, 16 TMA timeout, 32 overflow queue, 64 sort mismatch)", err);
+        char buf[220];
+        snprintf(buf, sizeof buf, "device fault word 0x%x (1 frame pool, 2 exchange buffer, 4 table pool, 8 moved >= 1 cell, 16 TMA timeout, 32 overflow queue, 64 sort mismatch, 128 species id outside the table)", err);
         return fail(c, PIC_EDEVICE, buf);
     }
     return PIC_OK;
@@ -389,6 +400,7 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     c->dt = dt;
     for (int a = 0; a < 3; ++a) c->cell[a] = cell[a];
     for (int s = 0; s < PIC_NSPECIES; ++s) { c->q[s] = -1.0; c->m[s] = 1.0; }
+    c->n_species = PIC_NSPECIES;
     c->max_particles = max_particles;
     c->n_particles = 0;
     c->steps = 0;
@@ -396,7 +408,6 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     c->stream = (cudaStream_t)stream;
     c->have_fields = false;
     c->use_tma = true;
-    c->use_graph = false;
     c->fuse_sort = true;
     c->cell_kernel = 0;
     c->field_update = false;
@@ -407,8 +418,6 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     c->force_class = -1;
     c->fixed_point = true;
     c->tmap_ok = false;
-    c->graph_exec = nullptr;
-    c->graph_steps = 0;
     c->timing = false;
     c->ws = (char*)workspace;
     c->ws_bytes = workspace_bytes;
@@ -470,8 +479,8 @@ int32_t pic_set_species(pic_ctx* c, int32_t n, const double* q, const double* m)
         if (!(m[s] > 0.0)) return fail(c, PIC_EINVAL, "pic_set_species: mass must be positive");
         c->q[s] = q[s]; c->m[s] = m[s];
     }
+    if (n > 0) c->n_species = n;      // particles of a species id >= n raise PIC_DEV_BAD_SPECIES when loaded
     refresh_species(c);
-    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
     return PIC_OK;
 }
 
@@ -629,6 +638,7 @@ int32_t pic_update_fields(pic_ctx* c)
 {
     if (!c) return PIC_EINVAL;
     if (!c->have_fields) return fail(c, PIC_ESTATE, "pic_update_fields: pic_set_fields has not been called");
+    if (!yee_stable(c)) return fail(c, PIC_EINVAL, "pic_update_fields: dt*sqrt(sum 1/cell^2) >= 1 (3-D Yee CFL limit)");
     cudaError_t e = enqueue_field_update(c, c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "pic_update_fields: launch");
     return PIC_OK;
@@ -737,7 +747,6 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
 {
     if (!c || !key) return PIC_EINVAL;
     if (!strcmp(key, "tma")) { c->use_tma = value != 0; return PIC_OK; }
-    if (!strcmp(key, "graph")) { c->use_graph = value != 0; return PIC_OK; }
     if (!strcmp(key, "class_all")) {
         if (value < -1 || value > 2) return fail(c, PIC_EINVAL, "pic_set_option: class_all must be in -1..2");
         c->force_class = (int)value;
@@ -749,7 +758,11 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
         c->cell_kernel = (int)value;
         return PIC_OK;
     }
-    if (!strcmp(key, "field_update")) { c->field_update = value != 0; return PIC_OK; }
+    if (!strcmp(key, "field_update")) {
+        if (value != 0 && !yee_stable(c)) return fail(c, PIC_EINVAL, "pic_set_option: field_update needs dt*sqrt(sum 1/cell^2) < 1 (3-D Yee CFL limit)");
+        c->field_update = value != 0;
+        return PIC_OK;
+    }
     if (!strcmp(key, "yee_index64")) { c->yee_index64 = value != 0; return PIC_OK; }
     if (!strcmp(key, "yee_tile")) {
         if (value != 8 && value != 16) return fail(c, PIC_EINVAL, "pic_set_option: yee_tile must be 8 or 16");
@@ -762,6 +775,16 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
         if (key[0] == 't') { c->d.two_phase = value != 0; return PIC_OK; }
         if (value < 2 || value > 16) return fail(c, PIC_EINVAL, "pic_set_option: segment must be in 2..16");
         c->d.seg_num = (int)value;
+        return PIC_OK;
+    }
+    // fault injection (tests): shrink a pool below what pic_workspace_bytes() sized it for, before any particle is
+    // loaded; the library must then raise the sticky device error instead of writing out of bounds
+    if (!strcmp(key, "limit_frames") || !strcmp(key, "limit_exchange") || !strcmp(key, "limit_tables")) {
+        if (c->n_particles > 0) return fail(c, PIC_ESTATE, "pic_set_option: set the limit_* options before loading particles");
+        if (value < 0) return fail(c, PIC_EINVAL, "pic_set_option: limit must be >= 0");
+        if (key[6] == 'f') c->d.n_frames = (int)(value < c->d.n_frames ? value : c->d.n_frames);
+        else if (key[6] == 'e') { c->d.x_cap = (int)(value < c->d.x_cap ? value : c->d.x_cap); }
+        else c->d.tbl_pool_size = (int)(value < c->d.tbl_pool_size ? value : c->d.tbl_pool_size);
         return PIC_OK;
     }
     if (!strcmp(key, "deposit")) { c->fixed_point = value != 0; return PIC_OK; }
@@ -795,7 +818,6 @@ const char* pic_last_error(const pic_ctx* c) { return c ? c->err.c_str() : g_cre
 int32_t pic_destroy(pic_ctx* c)
 {
     if (!c) return PIC_EINVAL;
-    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
     for (cudaEvent_t ev : c->events) cudaEventDestroy(ev);
     delete c;
     return PIC_OK;

@@ -623,7 +623,10 @@ __device__ __forceinline__ bool cell_is_dense(const PicDev& d, int s)
 {
     // the supercell's population: after the pending sort (fused prologue), or as sorted
     const int n = d.fused ? d.sc_next[s] : d.sc_count[s];
-    if (n == 0) return false;
+    if (n == 0) {
+        retire_empty_supercell(d, s);      // (called by one thread per supercell: thread 0 of its CTA, or the fetching thread)
+        return false;
+    }
     const bool sparse_class = d.class_all == 1 || (d.class_all == 0 && n < PIC_DIRECT_BELOW);
     return !sparse_class;
 }
@@ -636,7 +639,12 @@ pic_cell_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
     constexpr int NT = PIC_CELL_THREADS;
     using S = CellStage<O>;
     const int s = blockIdx.x;
-    if (!cell_is_dense(d, s)) return;
+    {
+        __shared__ int s_dense;
+        if (threadIdx.x == 0) s_dense = cell_is_dense(d, s);
+        __syncthreads();
+        if (!s_dense) return;
+    }
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const CellView<O> v(smem_raw);
     float4* s_stgP = reinterpret_cast<float4*>(smem_raw + S::BYTES);

@@ -50,7 +50,8 @@ struct PicDev {
     float jfx, jfy, jfz;         // (cell_a / dt) / (dx dy dz): J factor without q*w
     float h[PIC_NSPECIES];       // (q/m) dt / 2
     float q[PIC_NSPECIES];
-    float qmax;                  // max |q| over the species table
+    float qmax;                  // max |q| over the species slots in use
+    int n_species;               // species ids < n_species are valid
     // frames (two pools, see above)
     float4* rec[2];
     uint32_t* pid[2];

@@ -62,7 +62,10 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
     {
         // the supercell's population: after the pending sort (fused prologue), or as sorted
         const int n = d.fused ? d.sc_next[blockIdx.x] : d.sc_count[blockIdx.x];
-        if (n == 0) return;
+        if (n == 0) {
+            if (threadIdx.x == 0) retire_empty_supercell(d, blockIdx.x);
+            return;
+        }
         const bool sparse_class = d.class_all == 1 || (d.class_all == 0 && n < PIC_DIRECT_BELOW);
         if (sparse_class != SPARSE) return;
         if (!SPARSE) {

@@ -265,6 +265,14 @@ __device__ __forceinline__ void finish_particle(const PicDev& d, float4* rec, si
     }
 }
 
+// A supercell whose particles all left in the previous step (population after the pending sort = 0) is skipped by
+// every step kernel; when no stand-alone sort runs for it either (class_all == 2) its published count must still be
+// reset, or pic_prepare_kernel would build the next tail on the stale value.  Idempotent; one thread.
+__device__ __forceinline__ void retire_empty_supercell(const PicDev& d, int s)
+{
+    if (d.fused && d.sc_count[s] != 0) d.sc_count[s] = 0;
+}
+
 // Barrier over the NT threads that run a block-level routine: the whole CTA (BAR == 0, __syncthreads) or one warp
 // group of a warp-specialized kernel (named barrier BAR > 0; the other warps of the CTA do not take part).
 template <int BAR, int NT> __device__ __forceinline__ void group_sync()
