@@ -112,6 +112,19 @@ def compare(wl: W.Workload, orc: "oracle.Oracle", pic, n_steps: int, u_scale: fl
                         int((mism & near).sum()), bool(np.array_equal(cg, co)))
 
 
+def local_u_scale(wl: W.Workload, x, y, z, fields, n_steps: int, floor: float = 1e-3) -> np.ndarray:
+    """S17 for the laser case, per particle: the momentum tolerance is relative to max(|u|, u_scale) with
+    u_scale = |q/m| * F * dt/2, the momentum a particle at rest gains per step from the strongest field component F
+    within reach (the 3^3 cells around its start, widened by one cell per further step) — a0*dt/2 = 0.5 at the
+    centre of the pulse (reading D1), and the floor 1e-3 of S17 in the cold, field-free region."""
+    F = torch.as_tensor(np.asarray(fields)).abs().amax(0)[None, None].to(torch.float32)      # [1,1,nz,ny,nx]
+    r = n_steps
+    Fp = torch.nn.functional.pad(F, (r, r, r, r, r, r), mode="circular")
+    Fm = torch.nn.functional.max_pool3d(Fp, 2 * r + 1, stride=1)[0, 0].numpy()
+    ci = [np.floor(np.asarray(c) / wl.cell[a]).astype(np.int64) % wl.grid[a] for a, c in enumerate((x, y, z))]
+    return np.maximum(floor, 0.5 * wl.dt * Fm[ci[2], ci[1], ci[0]].astype(np.float64))
+
+
 def gpu_membership_consistent(wl: W.Workload, pic) -> bool:
     """Membership reported by the library == floor(X) div SC recomputed from its own positions."""
     P = pic.get_particles()
