@@ -31,6 +31,8 @@ struct pic_ctx {
     bool yee_index64;            // option "yee_index64": force the 64-bit-index instantiation (taken anyway beyond 2^32 elements)
     int yee_tile;                // option "yee_tile": y extent of the Yee kernel's tile (8 or 16)
     bool dirty;                  // pool cur holds a stepped state whose sort is still pending
+    bool sparse_float;           // option "sparse_float": all-sparse steps deposit in float (default on)
+    int crowd_min_on;            // PicDev::crowd_min when option "crowd_first" is on
     int force_class;             // option "class_all": -1 = from the counters (default), 0/1/2 = PicDev::class_all as given
     int max_known, min_known;    // largest / smallest non-empty supercell population as of the last synchronisation (0: unknown)
     int* hist[2];                // the two cell histograms; d.cell_hist == hist[hist_cur]
@@ -53,7 +55,7 @@ namespace {
 
 struct Layout {
     uint64_t rec0, rec1, pid0, pid1, free_stack, tbl_pool, tbl_off, tbl_cap, sc_nframes, sc_count, sc_tail, sc_incoming,
-        sc_left, sc_next, cell_off, cell_hist, cell_perm, cell_kbase, x_rec, x_id, x_dst, ovf, ctr, ctr64, F, F2, Fpad, J, J64, sc_offset, total;
+        sc_left, sc_next, sc_crowd, crowd_list, cell_off, cell_hist, cell_perm, cell_kbase, x_rec, x_id, x_dst, ovf, ctr, ctr64, F, F2, Fpad, J, J64, sc_offset, total;
     int n_frames, tbl_pool_size, x_cap, nsc;
 };
 
@@ -92,6 +94,8 @@ int compute_layout(const int32_t grid[3], const int32_t sc[3], int order, int64_
     L->sc_incoming = take(nsc * 4);
     L->sc_left = take(nsc * 4);
     L->sc_next = take(nsc * 4);
+    L->sc_crowd = take(nsc * 4);
+    L->crowd_list = take(PIC_CROWD_MAX * 4);
     L->cell_off = take(nsc * 257 * 4);
     L->cell_hist = take(2 * nsc * 256 * 4);      // two histograms (this step's, the previous step's)
     L->cell_perm = take(nsc * 256);
@@ -410,6 +414,7 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     c->use_tma = true;
     c->fuse_sort = true;
     c->cell_kernel = 0;
+    c->sparse_float = true;
     c->field_update = false;
     c->yee_tile = 8;
     c->yee_index64 = false;
@@ -444,6 +449,17 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     d.sc_nframes = (int*)(w + L.sc_nframes); d.sc_count = (int*)(w + L.sc_count);
     d.sc_tail = (int*)(w + L.sc_tail); d.sc_incoming = (int*)(w + L.sc_incoming);
     d.sc_left = (int*)(w + L.sc_left); d.sc_next = (int*)(w + L.sc_next);
+    d.sc_crowd = (int*)(w + L.sc_crowd); d.crowd_list = (int*)(w + L.crowd_list);
+    // crowded-first scheduling (option "crowd_first", off: measured slower): crowded = at least four times
+    // the mean population the context was sized for (and not below 8192)
+    {
+        const int64_t mean4 = 4 * (max_particles / (int64_t)L.nsc);
+        c->crowd_min_on = (int)(mean4 > 8192 ? (mean4 < (1 << 30) ? mean4 : (1 << 30)) : 8192);
+        d.crowd_min = 1 << 30;
+        d.direct_below = PIC_DIRECT_BELOW;
+        d.sparse_float_tile = 0;
+        d.float_tile_to_j64 = 0;
+    }
     d.fused = 0;
     d.class_all = 0;
     d.sort_filter = 0;
@@ -576,8 +592,18 @@ static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
             int rc = ensure_sorted(c);
             if (rc != PIC_OK) return rc;
         }
-        cudaError_t e = c->fixed_point ? cudaMemsetAsync(d.J64, 0, 3 * ncell * sizeof(long long), st)   // S16
-                                       : cudaMemsetAsync(d.J, 0, 3 * ncell * sizeof(float), st);
+        // which variants to launch: a belief from the last synchronisation, with a margin; a supercell that crossed
+        // the line since is still stepped correctly, by the variant that takes every supercell
+        d.class_all = 0;
+        if (c->max_known > 0 && c->max_known <= c->d.direct_below * 3 / 4) d.class_all = 1;
+        else if (c->min_known >= c->d.direct_below * 5 / 4) d.class_all = 2;
+        if (c->force_class >= 0) d.class_all = c->force_class;
+        // A step that only launches the sparse variant accumulates J in float (shared tile and global array): its
+        // supercells see few same-node collisions, and the 64-bit accumulators cost a memset and a convert pass over
+        // 3 x 8 B per CELL — on the 67 M-cell grid of configs[2] 4 GB per step, 17 % of the step (profiles/README.md)
+        const bool fix = c->fixed_point && !(c->sparse_float && d.class_all == 1);
+        cudaError_t e = fix ? cudaMemsetAsync(d.J64, 0, 3 * ncell * sizeof(long long), st)   // S16
+                            : cudaMemsetAsync(d.J, 0, 3 * ncell * sizeof(float), st);
         if (e == cudaSuccess) e = cudaMemsetAsync(d.ctr + CTR_EXCH, 0, sizeof(int), st);
         if (e == cudaSuccess) e = cudaMemsetAsync(d.ctr + CTR_OVF, 0, sizeof(int), st);
         if (e == cudaSuccess && c->cell_kernel == 2) e = cudaMemsetAsync(d.ctr + CTR_WORK, 0, sizeof(int), st);
@@ -587,12 +613,6 @@ static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
             if (e == cudaSuccess) e = cudaEventCreate(&ev1);
             if (e == cudaSuccess) e = cudaEventRecord(ev0, st);
         }
-        // which variants to launch: a belief from the last synchronisation, with a margin; a supercell that crossed
-        // the line since is still stepped correctly, by the variant that takes every supercell
-        d.class_all = 0;
-        if (c->max_known > 0 && c->max_known <= PIC_DIRECT_BELOW * 3 / 4) d.class_all = 1;
-        else if (c->min_known >= PIC_DIRECT_BELOW * 5 / 4) d.class_all = 2;
-        if (c->force_class >= 0) d.class_all = c->force_class;
         d.fused = c->dirty ? 1 : 0;
         if (c->dirty) d.cur ^= 1;       // the kernel sorts pool cur^1 into pool cur and steps it there
         d.cell_hist_prev = c->hist[c->hist_cur];        // pending histogram (all zero when the state is sorted)
@@ -605,15 +625,15 @@ static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
             ds.sort_filter = d.class_all == 1 ? 0 : 1;
             if (e == cudaSuccess) e = pic_launch_sort(ds, st, &c->launches);
         }
-        if (e == cudaSuccess) e = pic_launch_step(d, c->order, c->use_tma && c->tmap_ok, c->fixed_point, c->tmap, st, &c->launches, c->cell_kernel);
+        if (e == cudaSuccess) e = pic_launch_step(d, c->order, c->use_tma && c->tmap_ok, fix, c->tmap, st, &c->launches, c->cell_kernel);
         d.fused = 0;
         if (e == cudaSuccess && c->timing) {
             e = cudaEventRecord(ev1, st);
             c->events.push_back(ev0);
             c->events.push_back(ev1);
         }
-        if (e == cudaSuccess) e = pic_launch_overflow(d, c->order, c->fixed_point, st, &c->launches);
-        if (e == cudaSuccess && c->fixed_point) e = pic_launch_convert(d, st, &c->launches);
+        if (e == cudaSuccess) e = pic_launch_overflow(d, c->order, fix, st, &c->launches);
+        if (e == cudaSuccess && fix) e = pic_launch_convert(d, st, &c->launches);
         if (e == cudaSuccess) e = pic_launch_prepare(d, st, &c->launches);
         if (e == cudaSuccess) e = pic_launch_scatter(d, st, &c->launches);
         if (e == cudaSuccess && c->field_update) e = enqueue_field_update(c, st);
@@ -753,6 +773,15 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
         return PIC_OK;
     }
     if (!strcmp(key, "fuse_sort")) { c->fuse_sort = value != 0; return PIC_OK; }
+    if (!strcmp(key, "direct_below")) {
+        if (value < 1 || value > (1 << 20)) return fail(c, PIC_EINVAL, "pic_set_option: direct_below out of range");
+        if (c->n_particles > 0) return fail(c, PIC_ESTATE, "pic_set_option: set direct_below before loading particles");
+        c->d.direct_below = (int)value;
+        return PIC_OK;
+    }
+    if (!strcmp(key, "sparse_float_tile")) { c->d.sparse_float_tile = value != 0; return PIC_OK; }
+    if (!strcmp(key, "sparse_float")) { c->sparse_float = value != 0; return PIC_OK; }
+    if (!strcmp(key, "crowd_first")) { c->d.crowd_min = value ? c->crowd_min_on : (1 << 30); return PIC_OK; }
     if (!strcmp(key, "cell_kernel")) {
         if (value < 0 || value > 2) return fail(c, PIC_EINVAL, "pic_set_option: cell_kernel must be 0, 1 or 2");
         c->cell_kernel = (int)value;

@@ -627,7 +627,7 @@ __device__ __forceinline__ bool cell_is_dense(const PicDev& d, int s)
         retire_empty_supercell(d, s);      // (called by one thread per supercell: thread 0 of its CTA, or the fetching thread)
         return false;
     }
-    const bool sparse_class = d.class_all == 1 || (d.class_all == 0 && n < PIC_DIRECT_BELOW);
+    const bool sparse_class = d.class_all == 1 || (d.class_all == 0 && n < d.direct_below);
     return !sparse_class;
 }
 
@@ -638,7 +638,8 @@ pic_cell_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
 {
     constexpr int NT = PIC_CELL_THREADS;
     using S = CellStage<O>;
-    const int s = blockIdx.x;
+    const int s = pic_cta_supercell(d, blockIdx.x);
+    if (s < 0) return;
     {
         __shared__ int s_dense;
         if (threadIdx.x == 0) s_dense = cell_is_dense(d, s);
@@ -820,7 +821,7 @@ static cudaError_t launch_cell_one(const PicDev& d, const CUtensorMap& map, cuda
         if (ctas < 2) return cudaErrorLaunchOutOfResources;
         configured = true;
     }
-    pic_cell_kernel<O, TMA><<<d.nsc, PIC_CELL_THREADS, bytes, st>>>(d, map);
+    pic_cell_kernel<O, TMA><<<d.nsc + PIC_CROWD_MAX, PIC_CELL_THREADS, bytes, st>>>(d, map);
     return cudaGetLastError();
 }
 

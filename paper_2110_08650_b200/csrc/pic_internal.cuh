@@ -21,6 +21,7 @@
 #define PIC_SCZ 4
 #define PIC_SC_CELLS (PIC_SCX * PIC_SCY * PIC_SCZ)
 #define PIC_NSPECIES 16
+#define PIC_CROWD_MAX 1024       // CTAs in front of the step kernels' grids reserved for crowded supercells
 #define PIC_LEFT_FLAG 0x01000000u   // record bits: the particle left this supercell (hole until the sort)
 
 // device counters (int32 each) in PicDev::ctr
@@ -35,6 +36,7 @@ enum {
     CTR_OVF = 7,
     CTR_FREE_TOP = 8,     // entries on the stack of returned frames (may dip below 0 while prepare pops)          // entries in the overflow queue of out-of-window particles (this step)
        // bits of max |weight| loaded so far (non-negative floats order like ints)
+    CTR_CROWD = 11,       // entries in crowd_list (supercells the next step starts first), built by pic_prepare_kernel
     CTR_WORK = 10,        // next supercell of the persistent step kernel (zeroed before every launch)
     CTR_NEGMIN = 9,       // max over non-empty supercells of (2^30 - population) seen by pic_prepare_kernel, i.e. 2^30 - min
     CTR_N = 16
@@ -77,6 +79,12 @@ struct PicDev {
     int* sc_incoming;            // [nsc] leavers headed here
     int* sc_left;                // [nsc] leavers of the last step (written by the step kernel, consumed by prepare)
     int* sc_next;                // [nsc] population after the pending sort (stayers + arrivals), set by prepare
+    int* crowd_list;             // [PIC_CROWD_MAX] supercells with >= crowd_min particles: the step kernels start them first
+    int* sc_crowd;               // [nsc] 1 = listed in crowd_list (its natural CTA exits)
+    int crowd_min;
+    int sparse_float_tile;       // option "sparse_float_tile": the sparse variant keeps a float J tile (flushed into J64)
+    int float_tile_to_j64;       // set by the launcher for that variant
+    int direct_below;            // supercells with fewer particles count as sparse (one thread per particle); option "direct_below"
     int class_all;               // host's belief, from counters read at its last synchronisation (performance only, any
                                  // value is correct): 1 = no supercell is dense: the sparse variant takes every supercell;
                                  // 2 = none is sparse: the dense variant takes every supercell; 0 = classify by population
@@ -116,7 +124,7 @@ struct PicDev {
 // Two-phase path: an item's positions and gathered fields sit in shared memory, so an item holds at
 // most PIC_ITEM_LMAX particles (what fits beside the tiles with two CTAs per SM) and is flushed once.
 #define PIC_ITEM_LMAX(O) ((O) == 3 ? 6 : 11)
-#define PIC_DIRECT_BELOW 1536    // supercells with fewer particles (< 6 per cell) count as sparse: one thread per particle
+#define PIC_DIRECT_BELOW 768     // default of PicDev::direct_below: supercells with fewer particles (< 3 per cell) count as sparse
 #define PIC_ITEMCAP 1024         // work items per supercell: <= 256 + count/T
 
 // Work-item length target; lmax > 0 caps it where the supercell's item list still fits PIC_ITEMCAP
@@ -128,6 +136,17 @@ __host__ __device__ inline int pic_segment_target(int supercell_count, int seg_n
     if (t > 256) t = 256;      // PIC_FLUSH_MAX: the fixed-point split of a register sum is exact for <= 256 contributions
     if (lmax > 0 && supercell_count <= 768 * lmax) t = lmax;    // two-phase: items as long as the staging allows
     return t;
+}
+
+// Which supercell a step CTA works on: the first PIC_CROWD_MAX CTAs of the grid take the crowded supercells that
+// pic_prepare_kernel listed (one CTA walks 100 k particles while ordinary supercells take 4 k: started last, such a
+// CTA is the tail of the whole launch; started first, the others fill in around it), the rest their own index.
+// Returns -1 for a CTA without work.
+__device__ inline int pic_cta_supercell(const PicDev& d, int block)
+{
+    if (block < PIC_CROWD_MAX) return block < d.ctr[CTR_CROWD] ? d.crowd_list[block] : -1;
+    const int s = block - PIC_CROWD_MAX;
+    return d.sc_crowd[s] ? -1 : s;
 }
 
 __host__ __device__ inline uint32_t pic_pack_bits(int local_cell, int species)

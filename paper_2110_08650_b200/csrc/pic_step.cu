@@ -59,14 +59,16 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
     constexpr bool SPARSE = MODE == PIC_MODE_SPARSE;
     constexpr bool two_phase = MODE == PIC_MODE_TWO;
     constexpr int NT = SPARSE ? 256 : PIC_STEP_THREADS;
+    const int s = pic_cta_supercell(d, blockIdx.x);
+    if (s < 0) return;
     {
         // the supercell's population: after the pending sort (fused prologue), or as sorted
-        const int n = d.fused ? d.sc_next[blockIdx.x] : d.sc_count[blockIdx.x];
+        const int n = d.fused ? d.sc_next[s] : d.sc_count[s];
         if (n == 0) {
-            if (threadIdx.x == 0) retire_empty_supercell(d, blockIdx.x);
+            if (threadIdx.x == 0) retire_empty_supercell(d, s);
             return;
         }
-        const bool sparse_class = d.class_all == 1 || (d.class_all == 0 && n < PIC_DIRECT_BELOW);
+        const bool sparse_class = d.class_all == 1 || (d.class_all == 0 && n < d.direct_below);
         if (sparse_class != SPARSE) return;
         if (!SPARSE) {
             const bool fits_two = d.two_phase && pic_segment_target(n, d.seg_num, PIC_ITEM_LMAX(O)) <= PIC_ITEM_LMAX(O);
@@ -94,7 +96,6 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
     __shared__ __align__(8) uint64_t s_bar;
 
     const int tid = threadIdx.x;
-    const int s = blockIdx.x;
     const int ssx = s % d.nsx, ssy = (s / d.nsx) % d.nsy, ssz = s / (d.nsx * d.nsy);
     const int ox = ssx * PIC_SCX, oy = ssy * PIC_SCY, oz = ssz * PIC_SCZ;
     constexpr int NJ = (FIX ? 6 : 3) * G::JCOMP;
@@ -159,7 +160,7 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
     }
     // the item order: published by pic_sort_kernel for the supercells it counts as dense, else worked out here
     // (after the fused sort; or a supercell below the line that this variant takes under class_all == 2)
-    const bool own_order = fused || s_off[256] < PIC_DIRECT_BELOW;
+    const bool own_order = fused || s_off[256] < d.direct_below;
     if (!SPARSE && own_order) fused_item_order<NT>(tid, seg_T, s_off, s_w, s_bin, s_kcnt, s_perm, s_kb);
     if (!SPARSE)
     for (int t = tid; t < 256; t += NT) {
@@ -519,7 +520,16 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
                 if (n != 0) atomicAdd(reinterpret_cast<unsigned long long*>(d.J64) + g, (unsigned long long)n);
             } else {
                 const float v = sJ[e];
-                if (v != 0.0f) atomicAdd(d.J + g, v);
+                if (v == 0.0f) continue;
+                if (d.float_tile_to_j64) {
+                    // float tile of a sparse supercell (few same-node collisions: the CAS loop of a float atomic is
+                    // cheaper there than two integer atomics) into the fixed-point global accumulators
+                    const float jfc = c == 0 ? d.jfx : c == 1 ? d.jfy : d.jfz;
+                    const double scale = (double)fix_scale_of(d, jfc) * (double)(1 << PIC_FIX_LO_BITS);
+                    atomicAdd(reinterpret_cast<unsigned long long*>(d.J64) + g, (unsigned long long)__double2ll_rn((double)v * scale));
+                } else {
+                    atomicAdd(d.J + g, v);
+                }
             }
         }
     }
@@ -643,6 +653,15 @@ __global__ void pic_prepare_kernel(const PicDev d)
     d.sc_incoming[s] = 0;
     const int next = count - d.sc_left[s] + inc;
     d.sc_next[s] = next;                            // population after the pending sort
+    int listed = 0;
+    if (next >= d.crowd_min) {                      // crowded: the next step starts it first (pic_cta_supercell)
+        const int at = atomicAdd(d.ctr + CTR_CROWD, 1);
+        if (at < PIC_CROWD_MAX) {
+            d.crowd_list[at] = s;
+            listed = 1;
+        }
+    }
+    d.sc_crowd[s] = listed;
     d.sc_left[s] = 0;
     atomicMax(d.ctr + CTR_MAX_COUNT, count + inc);
     if (next > 0) atomicMax(d.ctr + CTR_NEGMIN, (1 << 30) - next);
@@ -682,8 +701,8 @@ __global__ void __launch_bounds__(PIC_FRAME) pic_sort_kernel(const PicDev d)
     __shared__ int s_wsum[8];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int s = blockIdx.x;
-    if (d.sort_filter && d.sc_next[s] >= PIC_DIRECT_BELOW) return;     // a dense step CTA sorts this one itself
-    const int n_scan = d.sc_tail[s];
+    if (d.sort_filter && d.sc_next[s] >= d.direct_below) return;     // a dense step CTA sorts this one itself
+    const int n_scan = min(d.sc_tail[s], d.sc_nframes[s] * PIC_FRAME);     // (see fused_sort: never beyond the owned frames)
     if (n_scan == 0) return;       // empty and nothing arrived: ranges, count and histogram are already zero
     const int cnt = d.cell_hist[(size_t)s * 256 + tid];
     d.cell_hist[(size_t)s * 256 + tid] = 0;
@@ -712,7 +731,7 @@ __global__ void __launch_bounds__(PIC_FRAME) pic_sort_kernel(const PicDev d)
     }
     // work items of the next step: cell c is cut into k = ceil(n/T) segments of ~n/k particles; order
     // the cells by decreasing segment length (ties by index) and publish the first item of each
-    if (total >= PIC_DIRECT_BELOW) {   // block-uniform; the per-particle path needs no work items
+    if (total >= d.direct_below) {   // block-uniform; the per-particle path needs no work items
     const int seg_T = pic_segment_target(total, d.seg_num, d.two_phase ? PIC_ITEM_LMAX(d.order) : 0);
     const int k = (cnt + seg_T - 1) / seg_T;
     const int seglen = k ? (cnt + k - 1) / k : 0;
@@ -826,7 +845,7 @@ static cudaError_t launch_step_one(const PicDev& d, const CUtensorMap& map, cuda
         if (ctas < 2) return cudaErrorLaunchOutOfResources;
         configured = true;
     }
-    pic_step_kernel<O, TMA, FIX, MODE><<<d.nsc, SPARSE ? 256 : PIC_STEP_THREADS, bytes, st>>>(d, map);
+    pic_step_kernel<O, TMA, FIX, MODE><<<d.nsc + PIC_CROWD_MAX, SPARSE ? 256 : PIC_STEP_THREADS, bytes, st>>>(d, map);
     return cudaGetLastError();
 }
 
@@ -847,7 +866,13 @@ static cudaError_t launch_step_variant(const PicDev& d, const CUtensorMap& map, 
         }
     }
     if (e == cudaSuccess && d.class_all != 2) {
-        e = launch_step_one<O, TMA, FIX, PIC_MODE_SPARSE>(d, map, st);
+        if (FIX && d.sparse_float_tile) {      // sparse supercells: float shared tile, fixed-point global accumulators
+            PicDev ds = d;
+            ds.float_tile_to_j64 = 1;
+            e = launch_step_one<O, TMA, false, PIC_MODE_SPARSE>(ds, map, st);
+        } else {
+            e = launch_step_one<O, TMA, FIX, PIC_MODE_SPARSE>(d, map, st);
+        }
         ++*launches;
     }
     return e;
@@ -898,6 +923,8 @@ cudaError_t pic_launch_convert(const PicDev& d, cudaStream_t st, int64_t* launch
 
 cudaError_t pic_launch_prepare(const PicDev& d, cudaStream_t st, int64_t* launches)
 {
+    cudaError_t e0 = cudaMemsetAsync(d.ctr + CTR_CROWD, 0, sizeof(int), st);      // the list is rebuilt by every prepare
+    if (e0 != cudaSuccess) return e0;
     pic_prepare_kernel<<<(d.nsc + 255) / 256, 256, 0, st>>>(d);
     ++*launches;
     return cudaGetLastError();

@@ -331,7 +331,9 @@ __device__ __forceinline__ int fused_sort(const PicDev& d, int s, int tid, int* 
                                           unsigned char* scratch = nullptr)
 {
     constexpr int PER = 256 / NT;
-    const int n_scan = d.sc_tail[s];
+    // slots in use, never beyond the frames the supercell owns (after a frame-pool fault the tail counts particles
+    // that found no slot: the table entries behind sc_nframes are not initialised)
+    const int n_scan = min(d.sc_tail[s], d.sc_nframes[s] * PIC_FRAME);
     int v[PER];
 #pragma unroll
     for (int k = 0; k < PER; ++k) {
