@@ -33,7 +33,8 @@ typedef struct {
     int32_t nx, ny, nz;      /* grid cells */
     int32_t scx, scy, scz;   /* supercell size in cells */
     int32_t order;           /* 1 CIC, 2 TSC, 3 PQS (polynomial degree, reading S2) */
-    int32_t reserved;
+    int32_t gather;          /* 0 momentum-conserving gather (reading S3, the contract's path); 1 energy-conserving
+                              * (Galerkin) gather: order o-1 along every axis a component is staggered on */
     double dx, dy, dz, dt;
 } orc_params;
 
@@ -51,6 +52,7 @@ static int orc_wrap(long i, int n) { long r = i % n; if (r < 0) r += n; return (
 double orc_shape(int order, double d)
 {
     double a = fabs(d);
+    if (order == 0) return (d >= -0.5 && d < 0.5) ? 1.0 : 0.0;   /* nearest grid point; a particle midway belongs to the upper node */
     if (order == 1) return a < 1.0 ? 1.0 - a : 0.0;
     if (order == 2) {
         if (a <= 0.5) return 0.75 - a * a;
@@ -73,8 +75,12 @@ double orc_gather_component(const orc_params* p, const double* F, const double s
     long b[3];
     double w[3][ORC_WN];
     for (int a = 0; a < 3; ++a) {
+        /* energy-conserving variant (8(f)2): one order lower along the axes this component is staggered on, so that a
+         * field that is the discrete gradient of a node potential is gathered as the exact gradient of the order-o
+         * interpolation of that potential: d/dx W_o(x - i) = W_{o-1}(x - (i - 1/2)) - W_{o-1}(x - (i + 1/2)) */
+        const int order = (p->gather == 1 && stag[a] != 0.0) ? p->order - 1 : p->order;
         b[a] = (long)floor(X[a] - stag[a]) + ORC_WLO;
-        for (int t = 0; t < ORC_WN; ++t) w[a][t] = orc_shape(p->order, X[a] - ((double)(b[a] + t) + stag[a]));
+        for (int t = 0; t < ORC_WN; ++t) w[a][t] = orc_shape(order, X[a] - ((double)(b[a] + t) + stag[a]));
     }
     double acc = 0.0;
     for (int c = 0; c < ORC_WN; ++c) {

@@ -22,14 +22,15 @@ _lib = None
 class OracleParams(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
                 ("scx", C.c_int32), ("scy", C.c_int32), ("scz", C.c_int32),
-                ("order", C.c_int32), ("reserved", C.c_int32),
+                ("order", C.c_int32), ("gather", C.c_int32),
                 ("dx", C.c_double), ("dy", C.c_double), ("dz", C.c_double), ("dt", C.c_double)]
 
     @staticmethod
-    def make(grid, cell=(1.0, 1.0, 1.0), dt=0.5, supercell=(8, 8, 4), order=1) -> "OracleParams":
+    def make(grid, cell=(1.0, 1.0, 1.0), dt=0.5, supercell=(8, 8, 4), order=1, gather=0) -> "OracleParams":
+        """gather: 0 momentum-conserving (the contract's path, S3), 1 energy-conserving / Galerkin."""
         return OracleParams(int(grid[0]), int(grid[1]), int(grid[2]),
                             int(supercell[0]), int(supercell[1]), int(supercell[2]),
-                            int(order), 0, float(cell[0]), float(cell[1]), float(cell[2]), float(dt))
+                            int(order), int(gather), float(cell[0]), float(cell[1]), float(cell[2]), float(dt))
 
 
 def build(force: bool = False) -> str:
@@ -142,8 +143,8 @@ class Oracle:
     """Stateful convenience wrapper mirroring the product's call sequence
     (create / set_species / load_particles / set_fields / step / get_*)."""
 
-    def __init__(self, grid, cell=(1.0, 1.0, 1.0), dt=0.5, supercell=(8, 8, 4), order=1):
-        self.prm = OracleParams.make(grid, cell, dt, supercell, order)
+    def __init__(self, grid, cell=(1.0, 1.0, 1.0), dt=0.5, supercell=(8, 8, 4), order=1, gather=0):
+        self.prm = OracleParams.make(grid, cell, dt, supercell, order, gather)
         self.q = np.full(256, -1.0)
         self.m = np.full(256, 1.0)
         self._parts = [np.zeros(0) for _ in range(7)]
