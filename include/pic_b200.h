@@ -177,6 +177,13 @@ int32_t pic_sync(pic_ctx* ctx);
  * most 11 particles — default, the fastest measured; 1 = pic_cell_kernel, one thread per cell; 2 = pic_pcell_kernel,
  * persistent CTAs whose producer warps sort and stage the next supercell beside the consumer warps; same results
  * within fp32 rounding of the per-cell sums; fixed-point deposit only),
+ * key "gather" (0 = momentum-conserving gather, every component at order o from its own staggered nodes — the contract's
+ * path, default; 1 = energy-conserving (Galerkin) gather: order o-1 along the
+ * axes a component is staggered on, so that a field -grad_h(phi) is gathered as the exact gradient of the order-o
+ * interpolation of phi; implemented in the kernels that gather per particle, hence it switches "two_phase" and
+ * "cell_kernel" to 0; only before the first pic_load_particles),
+ * key "direct_below" (default 768: supercells with fewer particles take the one-thread-per-particle variant),
+ * key "sparse_float" (1 = a step that only launches that variant accumulates J in float, default; 0 = always fixed point),
  * keys "limit_frames", "limit_exchange", "limit_tables" (fault injection for tests: lower the number of particle
  * frames / exchange-buffer entries / frame-table entries below what the workspace was sized for; only before the
  * first pic_load_particles; the step then raises PIC_DEV_FRAME_POOL_EXHAUSTED / PIC_DEV_EXCHANGE_OVERFLOW /

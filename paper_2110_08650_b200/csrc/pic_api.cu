@@ -457,6 +457,7 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
         c->crowd_min_on = (int)(mean4 > 8192 ? (mean4 < (1 << 30) ? mean4 : (1 << 30)) : 8192);
         d.crowd_min = 1 << 30;
         d.direct_below = PIC_DIRECT_BELOW;
+        d.gather_ec = 0;
         d.sparse_float_tile = 0;
         d.float_tile_to_j64 = 0;
     }
@@ -779,11 +780,21 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
         c->d.direct_below = (int)value;
         return PIC_OK;
     }
+    if (!strcmp(key, "gather")) {
+        // 1 = energy-conserving (Galerkin) gather: implemented in the kernels that gather per particle from the shared
+        // tile, so the dense supercells take the one-phase variant of pic_step.cu
+        if (value != 0 && value != 1) return fail(c, PIC_EINVAL, "pic_set_option: gather must be 0 or 1");
+        if (c->n_particles > 0) return fail(c, PIC_ESTATE, "pic_set_option: set gather before loading particles");
+        c->d.gather_ec = (int)value;
+        if (value) { c->d.two_phase = 0; c->cell_kernel = 0; }
+        return PIC_OK;
+    }
     if (!strcmp(key, "sparse_float_tile")) { c->d.sparse_float_tile = value != 0; return PIC_OK; }
     if (!strcmp(key, "sparse_float")) { c->sparse_float = value != 0; return PIC_OK; }
     if (!strcmp(key, "crowd_first")) { c->d.crowd_min = value ? c->crowd_min_on : (1 << 30); return PIC_OK; }
     if (!strcmp(key, "cell_kernel")) {
         if (value < 0 || value > 2) return fail(c, PIC_EINVAL, "pic_set_option: cell_kernel must be 0, 1 or 2");
+        if (value != 0 && c->d.gather_ec) return fail(c, PIC_EINVAL, "pic_set_option: gather = 1 needs cell_kernel = 0");
         c->cell_kernel = (int)value;
         return PIC_OK;
     }
@@ -801,7 +812,11 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
     if (!strcmp(key, "two_phase") || !strcmp(key, "segment")) {
         // the sorts publish the work-item layout from these two
         if (c->n_particles > 0) return fail(c, PIC_ESTATE, "pic_set_option: set two_phase / segment before loading particles");
-        if (key[0] == 't') { c->d.two_phase = value != 0; return PIC_OK; }
+        if (key[0] == 't') {
+            if (value != 0 && c->d.gather_ec) return fail(c, PIC_EINVAL, "pic_set_option: gather = 1 needs two_phase = 0");
+            c->d.two_phase = value != 0;
+            return PIC_OK;
+        }
         if (value < 2 || value > 16) return fail(c, PIC_EINVAL, "pic_set_option: segment must be in 2..16");
         c->d.seg_num = (int)value;
         return PIC_OK;

@@ -30,7 +30,10 @@ template <int O> struct Geo {
 // (SURVEY.md §8(c) step 1).  Returns the index of the first node with weight w[0].
 template <int O> __device__ __forceinline__ int shape(float xr, float (&w)[O + 1])
 {
-    if (O == 1) {
+    if (O == 0) {                        // nearest grid point (the staggered axes of the energy-conserving CIC gather)
+        w[0] = 1.0f;
+        return (int)floorf(xr + 0.5f);
+    } else if (O == 1) {
         float b = floorf(xr);
         float f = xr - b;
         w[0] = 1.0f - f;

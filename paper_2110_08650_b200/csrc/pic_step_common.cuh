@@ -142,9 +142,13 @@ __device__ __forceinline__ void flush2(float* sJ, int* sJhi, int* sJlo, int off0
 }
 
 // a2 for one particle: gather E,B at x^n from the shared tile.
+// ec = false: momentum-conserving gather (reading S3, the contract's path): order O on every axis.
+// ec = true: energy-conserving (Galerkin) gather: order O-1 along the axes a component is staggered
+//            on (the O weights are padded with a zero, so the same O+1-wide loops run; the extra node read lies
+//            inside the tile: it is a node the order-O window of a neighbouring position would touch).
 template <int O>
 __device__ __forceinline__ void gather_particle(const float* sF, int cx, int cy, int cz, const float4& P,
-                                                float (&E)[3], float (&B)[3])
+                                                float (&E)[3], float (&B)[3], bool ec = false)
 {
     using G = Geo<O>;
     {
@@ -154,7 +158,15 @@ __device__ __forceinline__ void gather_particle(const float* sF, int cx, int cy,
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
             bu[a] = shape<O>(f[a], wu[a]);
-            bs[a] = shape<O>(f[a] - 0.5f, ws[a]);
+            if (ec) {
+                float wl[O];
+                bs[a] = shape<O - 1>(f[a] - 0.5f, wl);
+#pragma unroll
+                for (int t = 0; t < O; ++t) ws[a][t] = wl[t];
+                ws[a][O] = 0.0f;
+            } else {
+                bs[a] = shape<O>(f[a] - 0.5f, ws[a]);
+            }
         }
         const int ux_ = cx + bu[0] + G::FL, sx_ = cx + bs[0] + G::FL;
         const int uy_ = (cy + bu[1] + G::FL) * G::FPX, sy_ = (cy + bs[1] + G::FL) * G::FPX;
@@ -218,7 +230,7 @@ __device__ __forceinline__ void push_particle(const PicDev& d, const float* sF, 
                                               float (&x1)[3], int (&sh)[3])
 {
     float E[3], B[3];
-    gather_particle<O>(sF, cx, cy, cz, P, E, B);
+    gather_particle<O>(sF, cx, cy, cz, P, E, B, d.gather_ec != 0);
     boris_move(d, sp, P, M, E, B, un, fn, x1, sh);
 }
 

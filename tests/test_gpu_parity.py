@@ -68,6 +68,37 @@ def test_dense_kernel_generations(name, kernel):
     pic.destroy()
 
 
+@pytest.mark.parametrize("name", ["cfg1_tiny_cic", "cfg2_thermal_tsc_32", "cfg3_lwfa_tsc_32x128x32", "cfg5_pqs_32x32x16"])
+def test_energy_conserving_gather_variant(name):
+    """Option gather = 1 against the oracle's energy-conserving gather (pinned in
+    tests/test_oracle_gather_ec.py): dense supercells through the one-phase kernel, sparse ones per particle."""
+    import oracle
+    wl, u_scale = CASES[name]
+    parts, fields = W.make_particles(wl), W.make_fields(wl)
+    if u_scale == "local":
+        u_scale = PP.local_u_scale(wl, parts.x.numpy(), parts.y.numpy(), parts.z.numpy(), fields.numpy(), 2)
+    orc = oracle.Oracle(wl.grid, wl.cell, wl.dt, wl.supercell, wl.shape_order, gather=1)
+    orc.load_particles(*(getattr(parts, k).numpy() for k in ("x", "y", "z", "ux", "uy", "uz", "w")),
+                       species=parts.species.numpy())
+    orc.set_fields(fields.numpy())
+    pic = PP.gpu_for(wl, parts, fields, gather=1)
+    assert orc.step(2) == 0
+    pic.step(2)
+    pic.sync()
+    rep = PP.compare(wl, orc, pic, 2, u_scale)
+    print(f"\n[{name} gather=1] {rep}")
+    assert rep.max_dx <= 2 * PP.TOL_X and rep.max_du_rel <= 2 * PP.TOL_U and rep.j_err_rel <= PP.TOL_J10
+    assert rep.n_member_mismatch == 0 and rep.counts_equal_outside_band
+    # and it is a different method: the momentum-conserving run differs by far more than the tolerance
+    ref = PP.gpu_for(wl, parts, fields)
+    ref.step(2)
+    A, B = PP.gpu_particles_by_id(pic), PP.gpu_particles_by_id(ref)
+    if name != "cfg1_tiny_cic":          # (uniform fields are gathered exactly by both)
+        assert np.abs(A["ux"] - B["ux"]).max() > 1e-5 * float(np.abs(B["ux"]).max() + 1e-3)
+    pic.destroy()
+    ref.destroy()
+
+
 @pytest.mark.parametrize("name", ["cfg1_tiny_cic", "cfg2_thermal_tsc_32", "cfg5_pqs_32x32x16"])
 def test_float_atomic_deposit_variant(name):
     """Option deposit=0 (float atomics on the shared J tile) computes the same step."""
