@@ -54,7 +54,7 @@ static std::string g_create_error;
 namespace {
 
 struct Layout {
-    uint64_t rec0, rec1, pid0, pid1, free_stack, tbl_pool, tbl_off, tbl_cap, sc_nframes, sc_count, sc_tail, sc_incoming,
+    uint64_t rec0, rec1, pid0, pid1, free_stack, tbl_pool, tbl_off, tbl_cap, tbl_old_off, tbl_old_cap, tbl_free, tbl_free_top, sc_nframes, sc_count, sc_tail, sc_incoming,
         sc_left, sc_next, sc_crowd, crowd_list, cell_off, cell_hist, cell_perm, cell_kbase, x_rec, x_id, x_dst, ovf, ctr, ctr64, F, F2, Fpad, J, J64, sc_offset, total;
     int n_frames, tbl_pool_size, x_cap, nsc;
 };
@@ -88,6 +88,10 @@ int compute_layout(const int32_t grid[3], const int32_t sc[3], int order, int64_
     L->tbl_pool = take(tblp * 4);
     L->tbl_off = take(nsc * 4);
     L->tbl_cap = take(nsc * 4);
+    L->tbl_old_off = take(nsc * 4);
+    L->tbl_old_cap = take(nsc * 4);
+    L->tbl_free = take((uint64_t)PIC_TBL_CLASSES * PIC_TBL_FREE * 4);
+    L->tbl_free_top = take(PIC_TBL_CLASSES * 4);
     L->sc_nframes = take(nsc * 4);
     L->sc_count = take(nsc * 4);
     L->sc_tail = take(nsc * 4);
@@ -446,6 +450,8 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     d.free_stack = (int*)(w + L.free_stack);
     d.tbl_pool = (int*)(w + L.tbl_pool); d.tbl_pool_size = L.tbl_pool_size;
     d.tbl_off = (int*)(w + L.tbl_off); d.tbl_cap = (int*)(w + L.tbl_cap);
+    d.tbl_old_off = (int*)(w + L.tbl_old_off); d.tbl_old_cap = (int*)(w + L.tbl_old_cap);
+    d.tbl_free = (int*)(w + L.tbl_free); d.tbl_free_top = (int*)(w + L.tbl_free_top);
     d.sc_nframes = (int*)(w + L.sc_nframes); d.sc_count = (int*)(w + L.sc_count);
     d.sc_tail = (int*)(w + L.sc_tail); d.sc_incoming = (int*)(w + L.sc_incoming);
     d.sc_left = (int*)(w + L.sc_left); d.sc_next = (int*)(w + L.sc_next);

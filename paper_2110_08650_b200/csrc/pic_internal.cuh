@@ -21,6 +21,8 @@
 #define PIC_SCZ 4
 #define PIC_SC_CELLS (PIC_SCX * PIC_SCY * PIC_SCZ)
 #define PIC_NSPECIES 16
+#define PIC_TBL_CLASSES 32
+#define PIC_TBL_FREE 2048        // free table regions remembered per capacity class
 #define PIC_CROWD_MAX 1024       // CTAs in front of the step kernels' grids reserved for crowded supercells
 #define PIC_LEFT_FLAG 0x01000000u   // record bits: the particle left this supercell (hole until the sort)
 
@@ -66,7 +68,11 @@ struct PicDev {
     int* tbl_pool;
     int tbl_pool_size;
     int* tbl_off;                // [nsc]
-    int* tbl_cap;                // [nsc]
+    int* tbl_cap;                // [nsc] capacity of the supercell's table region: 0 or a power of two >= 8
+    int* tbl_old_off;            // [nsc] region abandoned by the last growth (pushed on tbl_free by pic_scatter_kernel)
+    int* tbl_old_cap;            // [nsc] its capacity, 0 = none
+    int* tbl_free;               // [PIC_TBL_CLASSES][PIC_TBL_FREE] offsets of free regions by capacity class (log2)
+    int* tbl_free_top;           // [PIC_TBL_CLASSES] entries per class (prepare only pops, scatter only pushes)
     int* sc_nframes;             // [nsc]
     int* sc_count;               // [nsc] particles in the supercell
     int* sc_tail;                // [nsc] slots in use incl. holes of leavers and appended arrivals

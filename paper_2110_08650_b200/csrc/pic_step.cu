@@ -619,14 +619,36 @@ __global__ void pic_prepare_kernel(const PicDev d)
     int have = d.sc_nframes[s];
     if (need > have) {
         int off = d.tbl_off[s];
-        if (need > d.tbl_cap[s]) {           // grow the frame table (old region is abandoned)
-            const int ncap = max(2 * d.tbl_cap[s], need + 4);
-            const int noff = atomicAdd(d.ctr + CTR_TBL_TOP, ncap);
-            if (noff + ncap > d.tbl_pool_size) {
-                atomicOr(d.ctr + CTR_ERROR, PIC_DEV_TABLE_POOL_EXHAUSTED);
-                return;
+        if (need > d.tbl_cap[s]) {
+            // Grow the frame table: capacities are powers of two, a region of the right class is taken from the free
+            // lists if one is there (this kernel only pops — a CAS loop, no pushes run beside it — and
+            // pic_reclaim_tables_kernel, launched right after this one, only pushes), else cut from the pool.  The old region goes
+            // back to its class (a general allocator with reclaim).
+            const int ocap = d.tbl_cap[s];
+            int want = max(2 * ocap, need + 4), k = 3;
+            while ((1 << k) < want) ++k;
+            const int ncap = 1 << k;
+            int noff = -1;
+            for (int t = d.tbl_free_top[k]; t > 0;) {
+                const int seen = atomicCAS(d.tbl_free_top + k, t, t - 1);
+                if (seen == t) {
+                    noff = d.tbl_free[k * PIC_TBL_FREE + t - 1];
+                    break;
+                }
+                t = seen;
+            }
+            if (noff < 0) {
+                noff = atomicAdd(d.ctr + CTR_TBL_TOP, ncap);
+                if (noff + ncap > d.tbl_pool_size) {
+                    atomicOr(d.ctr + CTR_ERROR, PIC_DEV_TABLE_POOL_EXHAUSTED);
+                    return;
+                }
             }
             for (int i = 0; i < have; ++i) d.tbl_pool[noff + i] = d.tbl_pool[off + i];
+            if (ocap > 0) {
+                d.tbl_old_off[s] = off;
+                d.tbl_old_cap[s] = ocap;
+            }
             d.tbl_off[s] = off = noff;
             d.tbl_cap[s] = ncap;
         }
@@ -665,6 +687,22 @@ __global__ void pic_prepare_kernel(const PicDev d)
     d.sc_left[s] = 0;
     atomicMax(d.ctr + CTR_MAX_COUNT, count + inc);
     if (next > 0) atomicMax(d.ctr + CTR_NEGMIN, (1 << 30) - next);
+}
+
+// Table regions abandoned by the pic_prepare_kernel launched just before go back to the free list of their class
+// (push only; the next prepare pops).
+__global__ void pic_reclaim_tables_kernel(const PicDev d)
+{
+    for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < d.nsc; s += gridDim.x * blockDim.x) {
+        const int ocap = d.tbl_old_cap[s];
+        if (ocap == 0) continue;
+        int k = 3;
+        while ((1 << k) < ocap) ++k;
+        const int at = atomicAdd(d.tbl_free_top + k, 1);
+        if (at < PIC_TBL_FREE) d.tbl_free[k * PIC_TBL_FREE + at] = d.tbl_old_off[s];
+        else atomicSub(d.tbl_free_top + k, 1);          // list full: the region is lost (never handed out twice)
+        d.tbl_old_cap[s] = 0;
+    }
 }
 
 // One thread per leaver: claim a slot behind the destination's current slots (pool cur).
@@ -926,7 +964,8 @@ cudaError_t pic_launch_prepare(const PicDev& d, cudaStream_t st, int64_t* launch
     cudaError_t e0 = cudaMemsetAsync(d.ctr + CTR_CROWD, 0, sizeof(int), st);      // the list is rebuilt by every prepare
     if (e0 != cudaSuccess) return e0;
     pic_prepare_kernel<<<(d.nsc + 255) / 256, 256, 0, st>>>(d);
-    ++*launches;
+    pic_reclaim_tables_kernel<<<(d.nsc + 255) / 256, 256, 0, st>>>(d);
+    *launches += 2;
     return cudaGetLastError();
 }
 

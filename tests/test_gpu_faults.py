@@ -186,3 +186,37 @@ def test_emptied_supercell_with_every_variant_forced_dense(kernel):
     counts = pic.get_counts().cpu().numpy()
     assert counts[0] == 0 and counts.sum() == n
     pic.destroy()
+
+
+def test_frame_tables_are_reclaimed():
+    """a supercell that grows leaves its old frame-table region to the free list of its size class
+    and later growers take it from there.  Eight supercells are filled one after the other in four appending loads
+    each (tables of 16 -> 32 -> 64 entries): without reclaim that needs 8 x 112 = 896 table entries, with it
+    112 + 7 x 64 = 560; the pool is limited to 640."""
+    wl = W.CONFIGS["thermal_128"].scaled((16, 16, 8), ppc=1)
+    fields = W.make_fields(wl)
+    n_total = 8 * 12000
+    pic = Pic(wl.grid, wl.cell, wl.dt, wl.supercell, wl.shape_order, max_particles=n_total, device="cuda:0")
+    pic.set_option("limit_tables", 640)
+    g = torch.Generator().manual_seed(3)
+    loaded = 0
+    for k in range(8):
+        o = ((k % 2) * 8, ((k // 2) % 2) * 8, (k // 4) * 4)
+        for m in (1500, 1500, 3000, 6000):
+            r = torch.rand((3, m), generator=g, dtype=torch.float32).to(torch.float64)
+            x, y, z = o[0] + 8 * r[0], o[1] + 8 * r[1], o[2] + 4 * r[2]
+            u = 0.05 * torch.randn((3, m), generator=g)
+            pic.load_particles(x.cuda(), y.cuda(), z.cuda(), u[0].cuda(), u[1].cuda(), u[2].cuda(),
+                               torch.ones(m, device="cuda"), torch.zeros(m, dtype=torch.int32, device="cuda"))
+            loaded += m
+            pic.sync()                      # raises if the table pool ran dry
+    pic.set_fields(fields.cuda().contiguous())
+    pic.step(3)
+    pic.sync()
+    st = pic.get_stats()
+    assert st["error"] == 0 and st["particles"] == n_total == loaded
+    counts = pic.get_counts().cpu().numpy()
+    assert counts.sum() == n_total and counts.min() > 11000
+    ids = pic.get_particles()["id"].to(torch.int64) & 0xFFFFFFFF
+    assert torch.equal(torch.sort(ids).values, torch.arange(n_total, device="cuda"))
+    pic.destroy()
