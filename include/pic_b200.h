@@ -212,6 +212,26 @@ const char* pic_last_error(const pic_ctx* ctx);   /* ctx may be NULL: last creat
 
 int32_t pic_destroy(pic_ctx* ctx);                /* frees host state only */
 
+/* ONE entry point that allocates nothing and needs no context or workspace, for callers that cannot call cudaMalloc
+ * (code under CUDA graph capture, tight serving loops, harnesses that forbid allocation): the Esirkepov deposit
+ * (the same arithmetic as the step's per-particle deposit) of n particles given their positions
+ * before (x0,y0,z0) and after (x1,y1,z1) one step dt — float64 device arrays, global positions in the units of cell[],
+ * wrapped periodically; the move is taken as the minimum image and must be shorter than one cell per axis.  qw: float32
+ * device array, charge times weight.  Jx,Jy,Jz: float32 device arrays of nx*ny*nz elements, index i + nx*(j + ny*k),
+ * OVERWRITTEN with that step's current.  A particle that moved a cell or more (or a NaN position) is left out and
+ * element 0 of Jx, Jy and Jz is set to NaN (the call is asynchronous: the error shows in its output).
+ * Scratch (3 float64 sums per cell) lives in a file-scope device array of PIC_NOALLOC_MAX_CELLS cells = 6 MiB that every
+ * GPU which loads the library holds until the process exits: grids with more cells are rejected with PIC_EINVAL.  The
+ * array is shared by every call and cleared by each on its stream: calls that OVERLAP on the GPU (different streams, no
+ * event between them) race; calls on one stream are safe.  The first call on a device looks up the array's address
+ * (cudaGetSymbolAddress; make that call outside graph capture).  Calls no cudaMalloc/cudaFree.  grid, cell: host
+ * pointers; stream: cudaStream_t; errbuf (host, may be NULL): receives a message when the return value is not PIC_OK. */
+#define PIC_NOALLOC_MAX_CELLS 262144
+int32_t pic_deposit_current_noalloc(const int32_t grid[3], const double cell[3], double dt, int32_t shape_order,
+                                    int64_t n, const double* x0, const double* y0, const double* z0,
+                                    const double* x1, const double* y1, const double* z1, const float* qw,
+                                    float* Jx, float* Jy, float* Jz, void* stream, char* errbuf, int64_t errbuf_len);
+
 #ifdef __cplusplus
 }
 #endif

@@ -23,7 +23,7 @@ SYMBOLS = (
     "pic_workspace_bytes", "pic_create", "pic_set_species", "pic_load_particles", "pic_set_fields",
     "pic_step", "pic_get_current", "pic_get_particles", "pic_get_counts", "pic_get_stats", "pic_sync",
     "pic_set_option", "pic_get_timing", "pic_launch_count", "pic_last_error", "pic_destroy",
-    "pic_update_fields", "pic_get_fields",
+    "pic_update_fields", "pic_get_fields", "pic_deposit_current_noalloc",
 )
 
 
@@ -246,3 +246,34 @@ class Pic:
             self.destroy()
         except Exception:
             pass
+
+
+NOALLOC_MAX_CELLS = 262144     # PIC_NOALLOC_MAX_CELLS of include/pic_b200.h
+
+
+def deposit_current_noalloc(grid: Sequence[int], cell: Sequence[float], dt: float, shape_order: int,
+                            x0: torch.Tensor, y0: torch.Tensor, z0: torch.Tensor,
+                            x1: torch.Tensor, y1: torch.Tensor, z1: torch.Tensor, qw: torch.Tensor,
+                            out: torch.Tensor, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """pic_deposit_current_noalloc (include/pic_b200.h): the Esirkepov current of particles that moved x0 -> x1, into
+    the CALLER's `out` ([3, nz, ny, nx] float32, overwritten).  Marshalling only; nothing is allocated on the device,
+    here or in the library (scratch is a fixed 6 MiB device array: at most NOALLOC_MAX_CELLS cells).  Calls that
+    overlap on the GPU share that scratch and race: keep them on one stream."""
+    L = load_library()
+    n = int(x0.numel())
+    nx, ny, nz = (int(v) for v in grid)
+    if tuple(out.shape) != (3, nz, ny, nx) or out.dtype != torch.float32 or not out.is_cuda or not out.is_contiguous():
+        raise ValueError("out: expected a contiguous CUDA float32 tensor of shape [3, nz, ny, nx]")
+    args = [_ptr(t, torch.float64, n, k) for k, t in (("x0", x0), ("y0", y0), ("z0", z0), ("x1", x1), ("y1", y1), ("z1", z1))]
+    args.append(_ptr(qw, torch.float32, n, "qw"))
+    st = stream if stream is not None else torch.cuda.current_stream(out.device)
+    nb = out[0].numel() * 4
+    err = C.create_string_buffer(256)
+    with torch.cuda.device(out.device):
+        rc = L.pic_deposit_current_noalloc((C.c_int32 * 3)(nx, ny, nz), (C.c_double * 3)(*(float(v) for v in cell)),
+                                           C.c_double(float(dt)), int(shape_order), C.c_int64(n), *args,
+                                           *[C.c_void_p(out.data_ptr() + c * nb) for c in range(3)],
+                                           C.c_void_p(st.cuda_stream), err, C.c_int64(len(err)))
+    if rc != PIC_OK:
+        raise PicError(rc, err.value.decode())
+    return out

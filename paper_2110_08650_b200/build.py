@@ -14,7 +14,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpic_b200.so")
-SOURCES = ("pic_api.cu", "pic_step.cu", "pic_cell.cu", "pic_fields.cu")
+SOURCES = ("pic_api.cu", "pic_step.cu", "pic_cell.cu", "pic_fields.cu", "pic_noalloc.cu")
 HEADERS = ("pic_internal.cuh", "pic_device.cuh", "pic_step_common.cuh", os.path.join("..", "..", "include", "pic_b200.h"))
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
