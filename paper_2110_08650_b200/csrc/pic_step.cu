@@ -253,12 +253,19 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
         bool fits = true;
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
-            float w0[O + 1], w1[O + 1], s1[4];
-            const int b0 = shape<O>(f0[a], w0);
-            const int b1 = shape<O>(x1[a], w1);
-            fits &= (b1 >= -1) & (b1 <= 2 - O);
-            place4<O>(w0, b0 + 1, S0[a]);
-            place4<O>(w1, b1 + 1, s1);
+            float s1[4];
+            if constexpr (O == 2) {         // TSC: the window weights without floor / float->int / index compares
+                fits &= (x1[a] >= -0.5f) & (x1[a] < 1.5f);
+                tsc_window4(f0[a], S0[a]);
+                tsc_window4(x1[a], s1);
+            } else {
+                float w0[O + 1], w1[O + 1];
+                const int b0 = shape<O>(f0[a], w0);
+                const int b1 = shape<O>(x1[a], w1);
+                fits &= (b1 >= -1) & (b1 <= 2 - O);
+                place4<O>(w0, b0 + 1, S0[a]);
+                place4<O>(w1, b1 + 1, s1);
+            }
 #pragma unroll
             for (int t = 0; t < 4; ++t) DS[a][t] = s1[t] - S0[a][t];
         }
