@@ -471,9 +471,10 @@ def run_ours(args):
                          "frac_of_8000_GBps": achieved / 8000.0,
                          "kernel_share_of_step": kernel_ms_avg / (ms_max / K),
                          "binding_resource": "latency at 8 warps/SM (238 registers/thread, 114 KB shared memory per CTA): "
-                                             "0.47 instructions per cycle per scheduler, no pipe saturated (ncu: "
-                                             "profiles/README.md); HBM is the bound the metric names, not the one the "
-                                             "kernel hits",
+                                             "0.46 instructions per cycle per scheduler, FMA pipe 35 %, shared-memory pipe "
+                                             "61 % (ncu: profiles/r02_phase_budget.md); HBM is the bound the metric names, not "
+                                             "the one the kernel hits: its FP32 work alone is 0.94 ms per step (0.36 of the "
+                                             "roofline), its issue floor 1.27 ms",
                          "ncu": ncu_extra},
             "repeats": {"n": len(runs), "ms_per_step": [r[0] / K for r in runs], "headline": "median",
                         "each_from": "a freshly loaded state, warm-up steps first"},
