@@ -243,8 +243,12 @@ def measure_other(args, wl, dev, peak):
     pic = Pic(wl.grid, wl.cell, wl.dt, wl.supercell, wl.shape_order, max_particles=n, device=dev, workspace=ws)
     pic.set_option("cell_kernel", args.cell_kernel)
     pic.set_option("direct_below", args.direct_below)
+    pic.set_option("sparse_nosort", args.sparse_nosort)
     for k in ("tma", "deposit", "two_phase"):
         pic.set_option(k, getattr(args, k))
+    for kv in args.opt:
+        k, v = kv.split("=")
+        pic.set_option(k, int(v))
     for chunk in W.particle_chunks(wl, device=dev, max_chunk=1 << 23):
         pic.load_particles(chunk.x, chunk.y, chunk.z, chunk.ux, chunk.uy, chunk.uz, chunk.w, chunk.species)
         pic.sync()
@@ -325,8 +329,12 @@ def run_ours(args):
         pic.set_option("two_phase", args.two_phase)
         pic.set_option("cell_kernel", args.cell_kernel)
         pic.set_option("crowd_first", args.crowd_first)
+        pic.set_option("sparse_nosort", args.sparse_nosort)
         pic.set_option("direct_below", args.direct_below)
         pic.set_option("field_update", args.self_consistent)
+        for kv in args.opt:
+            k, v = kv.split("=")
+            pic.set_option(k, int(v))
         return pic
 
     # ---------------------------------------------------------------- device-resident throughput
@@ -503,6 +511,8 @@ def main():
     ap.add_argument("--two-phase", type=int, default=1, help="1: per-cell stencil in registers (two-phase items), 0: gather per particle from the shared tile")
     ap.add_argument("--cell-kernel", type=int, default=0, help="1: dense supercells go to pic_cell_kernel (third generation), 0: round-1 kernels")
     ap.add_argument("--direct-below", type=int, default=768, help="supercells with fewer particles take the per-particle (sparse) kernel")
+    ap.add_argument("--opt", action="append", default=[], help="key=value: any further pic_set_option (experiments)")
+    ap.add_argument("--sparse-nosort", type=int, default=1, help="1: all-sparse steps skip the re-sort (one sort in eight steps)")
     ap.add_argument("--crowd-first", type=int, default=0, help="1: the step kernels start crowded supercells first")
     ap.add_argument("--repeats", type=int, default=5, help="the headline is the median of this many runs, each from a fresh load")
     ap.add_argument("--late-run", type=int, default=1, help="1: also time the last 20 steps of the workload's own step count")

@@ -31,6 +31,8 @@ struct pic_ctx {
     bool yee_index64;            // option "yee_index64": force the 64-bit-index instantiation (taken anyway beyond 2^32 elements)
     int yee_tile;                // option "yee_tile": y extent of the Yee kernel's tile (8 or 16)
     bool dirty;                  // pool cur holds a stepped state whose sort is still pending
+    bool sparse_nosort;          // option "sparse_nosort": all-sparse steps skip the re-sort (default on)
+    int steps_unsorted;          // steps since the last sort
     bool sparse_float;           // option "sparse_float": all-sparse steps deposit in float (default on)
     int crowd_min_on;            // PicDev::crowd_min when option "crowd_first" is on
     int force_class;             // option "class_all": -1 = from the counters (default), 0/1/2 = PicDev::class_all as given
@@ -47,6 +49,8 @@ struct pic_ctx {
     bool timing;
     std::vector<cudaEvent_t> events;
 };
+
+#define PIC_NOSORT_PERIOD 8       // all-sparse steps: one sort in this many steps
 
 static std::string g_create_error;
 
@@ -419,6 +423,8 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     c->fuse_sort = true;
     c->cell_kernel = 0;
     c->sparse_float = true;
+    c->sparse_nosort = true;
+    c->steps_unsorted = 0;
     c->field_update = false;
     c->yee_tile = 8;
     c->yee_index64 = false;
@@ -464,6 +470,7 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
         d.crowd_min = 1 << 30;
         d.direct_below = PIC_DIRECT_BELOW;
         d.gather_ec = 0;
+        d.nosort = 0;
         d.sparse_float_tile = 0;
         d.float_tile_to_j64 = 0;
     }
@@ -570,6 +577,8 @@ static int ensure_sorted(pic_ctx* c)
 {
     if (!c->dirty) return PIC_OK;
     c->d.fused = 0;
+    c->d.nosort = 0;
+    c->steps_unsorted = 0;
     cudaError_t e = pic_launch_sort(c->d, c->stream, &c->launches);
     if (e != cudaSuccess) return cuda_fail(c, e, "sort");
     c->d.cur ^= 1;
@@ -620,12 +629,27 @@ static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
             if (e == cudaSuccess) e = cudaEventCreate(&ev1);
             if (e == cudaSuccess) e = cudaEventRecord(ev0, st);
         }
+        // An all-sparse step needs no cell order (one thread per particle): it can run on the unsorted state the last
+        // step left — holes of leavers, arrivals appended — instead of re-sorting 100 % of the records when a fraction of
+        // a percent moved; a sort every PIC_NOSORT_PERIOD steps bounds the holes.
+        const bool nosort = c->sparse_nosort && c->dirty && c->fuse_sort && d.class_all == 1 &&
+                            c->steps_unsorted < PIC_NOSORT_PERIOD;
+        d.nosort = nosort ? 1 : 0;
         d.fused = c->dirty ? 1 : 0;
-        if (c->dirty) d.cur ^= 1;       // the kernel sorts pool cur^1 into pool cur and steps it there
-        d.cell_hist_prev = c->hist[c->hist_cur];        // pending histogram (all zero when the state is sorted)
-        c->hist_cur ^= 1;
-        d.cell_hist = c->hist[c->hist_cur];             // this step's
-        if (d.fused && d.class_all != 2) {      // sparse supercells: the stand-alone sort, from the other pool into this one
+        if (nosort) {
+            // the pending histogram is not consumed by a sort: clear it and let this step fill it again
+            if (e == cudaSuccess) e = pic_launch_zero_ints(c->hist[c->hist_cur], (size_t)d.nsc * 256, st, &c->launches);
+            d.cell_hist = c->hist[c->hist_cur];
+            d.cell_hist_prev = c->hist[c->hist_cur ^ 1];
+            ++c->steps_unsorted;
+        } else {
+            if (c->dirty) d.cur ^= 1;       // the kernel sorts pool cur^1 into pool cur and steps it there
+            d.cell_hist_prev = c->hist[c->hist_cur];        // pending histogram (all zero when the state is sorted)
+            c->hist_cur ^= 1;
+            d.cell_hist = c->hist[c->hist_cur];             // this step's
+            c->steps_unsorted = 0;
+        }
+        if (!nosort && d.fused && d.class_all != 2) {      // sparse supercells: the stand-alone sort, from the other pool into this one
             PicDev ds = d;
             ds.cur = d.cur ^ 1;
             ds.cell_hist = d.cell_hist_prev;
@@ -643,6 +667,7 @@ static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
         if (e == cudaSuccess && fix) e = pic_launch_convert(d, st, &c->launches);
         if (e == cudaSuccess) e = pic_launch_prepare(d, st, &c->launches);
         if (e == cudaSuccess) e = pic_launch_scatter(d, st, &c->launches);
+        d.nosort = 0;
         if (e == cudaSuccess && c->field_update) e = enqueue_field_update(c, st);
         if (e != cudaSuccess) return cuda_fail(c, e, "pic_step: launch");
         c->dirty = true;
@@ -797,6 +822,7 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
     }
     if (!strcmp(key, "sparse_float_tile")) { c->d.sparse_float_tile = value != 0; return PIC_OK; }
     if (!strcmp(key, "sparse_float")) { c->sparse_float = value != 0; return PIC_OK; }
+    if (!strcmp(key, "sparse_nosort")) { c->sparse_nosort = value != 0; return PIC_OK; }
     if (!strcmp(key, "crowd_first")) { c->d.crowd_min = value ? c->crowd_min_on : (1 << 30); return PIC_OK; }
     if (!strcmp(key, "cell_kernel")) {
         if (value < 0 || value > 2) return fail(c, PIC_EINVAL, "pic_set_option: cell_kernel must be 0, 1 or 2");

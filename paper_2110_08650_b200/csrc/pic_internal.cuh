@@ -90,6 +90,7 @@ struct PicDev {
     int crowd_min;
     int sparse_float_tile;       // option "sparse_float_tile": the sparse variant keeps a float J tile (flushed into J64)
     int float_tile_to_j64;       // set by the launcher for that variant
+    int nosort;                  // this step runs on the unsorted state of the last one (all-sparse steps, option "sparse_nosort")
     int gather_ec;               // option "gather" = 1: energy-conserving gather (per-particle gather paths only)
     int direct_below;            // supercells with fewer particles count as sparse (one thread per particle); option "direct_below"
     int class_all;               // host's belief, from counters read at its last synchronisation (performance only, any
@@ -169,6 +170,7 @@ cudaError_t pic_launch_cell(const PicDev& d, int order, bool use_tma, const void
                             bool persistent);
 cudaError_t pic_launch_overflow(const PicDev& d, int order, bool fixed_point, cudaStream_t st, int64_t* launches);
 cudaError_t pic_launch_convert(const PicDev& d, cudaStream_t st, int64_t* launches);
+cudaError_t pic_launch_zero_ints(int* p, size_t n, cudaStream_t st, int64_t* launches);   // n a multiple of 4
 cudaError_t pic_launch_prepare(const PicDev& d, cudaStream_t st, int64_t* launches);
 cudaError_t pic_launch_scatter(const PicDev& d, cudaStream_t st, int64_t* launches);
 cudaError_t pic_launch_sort(const PicDev& d, cudaStream_t st, int64_t* launches);   // pool cur -> the other

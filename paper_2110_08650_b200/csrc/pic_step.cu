@@ -203,20 +203,27 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
     const int n_items = s_nitems;
     constexpr int SX = 1, SY = G::JNX, SZ = G::JNX * G::JNY;
 
-    const int count = s_off[256];
+    // (no-sort step, sparse variant only: the slots in use — stayers, holes of earlier leavers, appended arrivals —
+    // are walked as they are; the variant needs no cell order)
+    const int count = (SPARSE && d.nosort) ? min(d.sc_tail[s], d.sc_nframes[s] * PIC_FRAME) : s_off[256];
     if (SPARSE) {
         // sparse supercell (a few particles per cell): register sums would be flushed almost once per
         // particle, so take one thread per particle, coalesced, and deposit straight into the tile
         for (int base = 0; base < count; base += NT) {
             if (base + (tid & ~31) >= count) continue;       // warp-uniform
             const int slot = base + tid;
-            const bool active = slot < count;
+            bool active = slot < count;
             float4 P = make_float4(0.5f, 0.5f, 0.5f, 0.0f), M = make_float4(0.f, 0.f, 0.f, 0.f);   // ghost lane
             size_t idx = 0;
             if (active) {
                 idx = (size_t)tbl[slot >> 8] * PIC_FRAME + (slot & (PIC_FRAME - 1));
                 P = rec[2 * idx];
                 M = rec[2 * idx + 1];
+                if (__float_as_uint(M.w) & PIC_LEFT_FLAG) {      // hole of a particle that left in an earlier step
+                    active = false;
+                    P = make_float4(0.5f, 0.5f, 0.5f, 0.0f);
+                    M = make_float4(0.f, 0.f, 0.f, 0.f);
+                }
             }
             const uint32_t bits = __float_as_uint(M.w);
             const int lc = bits & 0xff, sp = (bits >> 16) & 0xff;
@@ -620,7 +627,9 @@ __global__ void pic_prepare_kernel(const PicDev d)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= d.nsc) return;
-    const int count = d.sc_count[s];
+    // slots in use: the sorted population, or — after a step that ran without a sort — everything up to the tail
+    // (holes stay until the next sort; arrivals are appended behind them)
+    const int count = d.nosort ? d.sc_tail[s] : d.sc_count[s];
     const int inc = d.sc_incoming[s];
     const int need = (count + inc + PIC_FRAME - 1) / PIC_FRAME;
     int have = d.sc_nframes[s];
@@ -680,7 +689,7 @@ __global__ void pic_prepare_kernel(const PicDev d)
     }
     d.sc_tail[s] = count;
     d.sc_incoming[s] = 0;
-    const int next = count - d.sc_left[s] + inc;
+    const int next = (d.nosort ? d.sc_next[s] : count) - d.sc_left[s] + inc;
     d.sc_next[s] = next;                            // population after the pending sort
     int listed = 0;
     if (next >= d.crowd_min) {                      // crowded: the next step starts it first (pic_cta_supercell)
@@ -692,7 +701,8 @@ __global__ void pic_prepare_kernel(const PicDev d)
     }
     d.sc_crowd[s] = listed;
     d.sc_left[s] = 0;
-    atomicMax(d.ctr + CTR_MAX_COUNT, count + inc);
+    // (largest population seen: particles, not slots — after a step without a sort `count` includes the holes)
+    atomicMax(d.ctr + CTR_MAX_COUNT, (d.nosort ? next : count + inc));
     if (next > 0) atomicMax(d.ctr + CTR_NEGMIN, (1 << 30) - next);
 }
 
@@ -955,6 +965,19 @@ cudaError_t pic_launch_overflow(const PicDev& d, int order, bool fixed_point, cu
         case 6: pic_overflow_kernel<3, false><<<g, b, 0, st>>>(d); break;
         default: pic_overflow_kernel<3, true><<<g, b, 0, st>>>(d); break;
     }
+    ++*launches;
+    return cudaGetLastError();
+}
+
+__global__ void pic_zero_ints_kernel(int4* p, size_t n16)
+{
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n16; i += (size_t)gridDim.x * blockDim.x)
+        p[i] = make_int4(0, 0, 0, 0);
+}
+
+cudaError_t pic_launch_zero_ints(int* p, size_t n, cudaStream_t st, int64_t* launches)
+{
+    pic_zero_ints_kernel<<<148 * 8, 256, 0, st>>>(reinterpret_cast<int4*>(p), n / 4);     // n is a multiple of 256
     ++*launches;
     return cudaGetLastError();
 }

@@ -99,6 +99,29 @@ def test_energy_conserving_gather_variant(name):
     ref.destroy()
 
 
+@pytest.mark.parametrize("nosort", (0, 1))
+def test_all_sparse_steps_without_resort(nosort):
+    """All-sparse workload (2 particles per cell, one thread per particle): with option sparse_nosort the steps run on
+    the unsorted state (holes of leavers, appended arrivals) and sort once in eight steps.  20 free-running steps of a
+    hot, sparse plasma (a few per cent of the particles change supercell per step, whole supercells of the slab
+    boundary empty and fill) against the oracle, with and without the option; read-backs in between sort on demand."""
+    wl = W.CONFIGS["lwfa"].scaled((32, 64, 16), u_th=0.25, ramp_cells=8)
+    parts, fields = W.make_particles(wl), W.make_fields(wl) * 0.02
+    orc = PP.oracle_for(wl, parts, fields)
+    pic = PP.gpu_for(wl, parts, fields, sparse_nosort=nosort)
+    for n in (3, 9, 8):
+        assert orc.step(n) == 0
+        pic.step(n)
+        pic.sync()
+        assert PP.gpu_membership_consistent(wl, pic)       # sorts the pending state for the read-back
+    rep = PP.compare(wl, orc, pic, 20, 0.25)
+    print(f"\n[all-sparse, sparse_nosort={nosort}] {rep} leavers={pic.get_stats()['leavers_cum']}")
+    assert pic.get_stats()["error"] == 0 and pic.get_stats()["leavers_cum"] > parts.n // 4
+    assert rep.max_dx <= 20 * PP.TOL_X and rep.max_du_rel <= 20 * PP.TOL_U and rep.j_err_rel <= PP.TOL_J10
+    assert rep.n_member_mismatch == 0 and rep.counts_equal_outside_band
+    pic.destroy()
+
+
 @pytest.mark.parametrize("name", ["cfg1_tiny_cic", "cfg2_thermal_tsc_32", "cfg5_pqs_32x32x16"])
 def test_float_atomic_deposit_variant(name):
     """Option deposit=0 (float atomics on the shared J tile) computes the same step."""
