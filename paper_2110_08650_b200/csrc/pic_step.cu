@@ -232,7 +232,11 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
             int sh[3];
             push_particle<O>(d, sF, cx, cy, cz, sp, P, M, un, fn, x1, sh);
             const float f0[3] = {P.x, P.y, P.z};
-            deposit_direct<O, FIX>(d, sJ, sJhi, sJlo, fix_scale, f0, x1, d.q[sp] * P.w, lc);
+            // a particle whose position did not change in fp32 deposits exactly nothing (every DS is 0): a warp of
+            // such particles (cold plasma ahead of a laser pulse) skips the deposit altogether
+            const bool moved = (x1[0] != f0[0]) | (x1[1] != f0[1]) | (x1[2] != f0[2]);
+            if (__any_sync(0xffffffffu, moved))
+                deposit_direct<O, FIX>(d, sJ, sJhi, sJlo, fix_scale, f0, x1, d.q[sp] * P.w, lc);
             if (active)
                 finish_particle(d, rec, idx, s, ssx, ssy, ssz, cx, cy, cz, sp, P, M, un, fn, sh, s_hist, &s_xn, s_xrec,
                                 s_xid, s_xdst);
