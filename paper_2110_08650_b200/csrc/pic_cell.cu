@@ -145,13 +145,7 @@ __device__ __forceinline__ void accumulate_pairs(f32x2 (&A)[3][2][4], float fac,
     }
 }
 
-// a5 for one particle, as finish_particle (pic_step_common.cuh) but a stayer's record goes back as ONE 32-byte
-// store (st.global.v8.f32, SASS STG.E.ENL2.256): half the store wavefronts of two 16-byte halves.
-__device__ __forceinline__ void store_record256(float4* dst, const float4& P, const float4& M)
-{
-    asm volatile("st.global.v8.f32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
-                 :: "l"(dst), "f"(P.x), "f"(P.y), "f"(P.z), "f"(P.w), "f"(M.x), "f"(M.y), "f"(M.z), "f"(M.w) : "memory");
-}
+// a5 for one particle, as finish_particle (pic_step_common.cuh) with the 32-byte store of store_record256
 __device__ __forceinline__ void finish_particle256(const PicDev& d, float4* rec, size_t idx, int ssx, int ssy, int ssz,
                                                    int cx, int cy, int cz, int sp, float4 P, float4 M,
                                                    const float (&un)[3], const float (&fn)[3], const int (&sh)[3],

@@ -217,8 +217,7 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
             size_t idx = 0;
             if (active) {
                 idx = (size_t)tbl[slot >> 8] * PIC_FRAME + (slot & (PIC_FRAME - 1));
-                P = rec[2 * idx];
-                M = rec[2 * idx + 1];
+                load_record256(rec + 2 * idx, P, M);
                 if (__float_as_uint(M.w) & PIC_LEFT_FLAG) {      // hole of a particle that left in an earlier step
                     active = false;
                     P = make_float4(0.5f, 0.5f, 0.5f, 0.0f);
@@ -522,15 +521,18 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
     // ---- a4: flush the J tile once (periodic wrap on write)
     {
         const size_t ncell = (size_t)d.nx * d.ny * d.nz;
-        for (int e = tid; e < 3 * G::JCOMP; e += NT) {
-            int i = e % G::JNX;
-            int r = e / G::JNX;
-            int j = r % G::JNY;
-            r /= G::JNY;
-            int k = r % G::JNZ;
-            int c = r / G::JNZ;
-            int gi = wrapi(ox + i - G::JL, d.nx), gj = wrapi(oy + j - G::JL, d.ny),
-                gk = wrapi(oz + k - G::JL, d.nz);
+        // 16 lanes per tile row of JNX <= 13 nodes: the row's y/z wrap and component are worked out once per row
+        constexpr int ROWS = 3 * G::JNZ * G::JNY;
+        const int i = tid & 15;
+        const int gi = wrapi(ox + i - G::JL, d.nx);
+        if (i < G::JNX)
+        for (int row = tid >> 4; row < ROWS; row += NT / 16) {
+            const int e = row * G::JNX + i;
+            const int j = row % G::JNY;
+            const int r2 = row / G::JNY;
+            const int k = r2 % G::JNZ;
+            const int c = r2 / G::JNZ;
+            const int gj = wrapi(oy + j - G::JL, d.ny), gk = wrapi(oz + k - G::JL, d.nz);
             const size_t g = c * ncell + (size_t)gi + (size_t)d.nx * ((size_t)gj + (size_t)d.ny * gk);
             if (FIX) {
                 // 64-bit fixed point in global memory too (native RED.64 in L2)
@@ -851,8 +853,7 @@ __global__ void __launch_bounds__(PIC_FRAME) pic_sort_kernel(const PicDev d)
 #pragma unroll
         for (int u = 0; u < U; ++u)
             if (ok[u]) {
-                P[u] = src[2 * i[u]];
-                M[u] = src[2 * i[u] + 1];
+                load_record256(src + 2 * i[u], P[u], M[u]);
                 id[u] = sid[i[u]];
             }
 #pragma unroll
@@ -866,8 +867,7 @@ __global__ void __launch_bounds__(PIC_FRAME) pic_sort_kernel(const PicDev d)
                 continue;
             }
             const size_t o = (size_t)tbl[r >> 8] * PIC_FRAME + (r & (PIC_FRAME - 1));
-            dst[2 * o] = P[u];
-            dst[2 * o + 1] = M[u];
+            store_record256(dst + 2 * o, P[u], M[u]);
             did[o] = id[u];
         }
     }

@@ -234,6 +234,20 @@ __device__ __forceinline__ void push_particle(const PicDev& d, const float* sF, 
     boris_move(d, sp, P, M, E, B, un, fn, x1, sh);
 }
 
+// One record = one 32-byte DRAM sector, written back as ONE store (st.global.v8.f32, SASS STG.E.ENL2.256): half the
+// store instructions and L1 wavefronts of two 16-byte halves.
+__device__ __forceinline__ void store_record256(float4* dst, const float4& P, const float4& M)
+{
+    asm volatile("st.global.v8.f32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
+                 :: "l"(dst), "f"(P.x), "f"(P.y), "f"(P.z), "f"(P.w), "f"(M.x), "f"(M.y), "f"(M.z), "f"(M.w) : "memory");
+}
+
+__device__ __forceinline__ void load_record256(const float4* src, float4& P, float4& M)
+{
+    asm volatile("ld.global.v8.f32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=f"(P.x), "=f"(P.y), "=f"(P.z), "=f"(P.w), "=f"(M.x), "=f"(M.y), "=f"(M.z), "=f"(M.w) : "l"(src) : "memory");
+}
+
 // a5 for one particle: new local cell and destination supercell; stayers are written back in place
 // and counted per new cell, leavers leave a flagged hole and are staged for the exchange buffer.
 __device__ __forceinline__ void finish_particle(const PicDev& d, float4* rec, size_t idx, int s, int ssx, int ssy, int ssz,
@@ -254,8 +268,7 @@ __device__ __forceinline__ void finish_particle(const PicDev& d, float4* rec, si
     M.x = unx; M.y = uny; M.z = unz;
     if ((dsx | dsy | dsz) == 0) {
         M.w = __uint_as_float(nbits);
-        rec[2 * idx] = P;
-        rec[2 * idx + 1] = M;
+        store_record256(rec + 2 * idx, P, M);
         atomicAdd(&s_hist[nlc], 1);
     } else {
         const int dst = wrapi(ssx + dsx, d.nsx) + d.nsx * (wrapi(ssy + dsy, d.nsy) + d.nsy * wrapi(ssz + dsz, d.nsz));
@@ -429,8 +442,7 @@ __device__ __forceinline__ int fused_sort(const PicDev& d, int s, int tid, int* 
             q.ok[u] = slot < n_scan;
             if (q.ok[u]) {
                 const size_t i = (size_t)tbl[slot >> 8] * PIC_FRAME + (slot & (PIC_FRAME - 1));
-                q.P[u] = __ldcs(src + 2 * i);
-                q.M[u] = __ldcs(src + 2 * i + 1);
+                load_record256(src + 2 * i, q.P[u], q.M[u]);
                 q.id[u] = __ldcs(sid + i);
             }
         }
@@ -447,8 +459,7 @@ __device__ __forceinline__ int fused_sort(const PicDev& d, int s, int tid, int* 
                 continue;
             }
             const size_t o = (size_t)tbl[r >> 8] * PIC_FRAME + (r & (PIC_FRAME - 1));
-            dst[2 * o] = q.P[u];
-            dst[2 * o + 1] = q.M[u];
+            store_record256(dst + 2 * o, q.P[u], q.M[u]);
             did[o] = q.id[u];
         }
     };
