@@ -36,6 +36,7 @@ struct pic_ctx {
     bool sparse_float;           // option "sparse_float": all-sparse steps deposit in float (default on)
     int crowd_min_on;            // PicDev::crowd_min when option "crowd_first" is on
     int force_class;             // option "class_all": -1 = from the counters (default), 0/1/2 = PicDev::class_all as given
+    int n_dense, n_sparse;       // non-empty supercells on either side of the sparse/dense line at the last synchronisation
     int max_known, min_known;    // largest / smallest non-empty supercell population as of the last synchronisation (0: unknown)
     int* hist[2];                // the two cell histograms; d.cell_hist == hist[hist_cur]
     int hist_cur;
@@ -335,6 +336,8 @@ int check_device(pic_ctx* c)
     const int err = ctr[CTR_ERROR];
     // populations seen so far (running max / min): lets the next steps skip kernel variants no supercell needs
     c->max_known = ctr[CTR_MAX_COUNT];
+    c->n_dense = ctr[CTR_NDENSE];
+    c->n_sparse = ctr[CTR_NSPARSE];
     c->min_known = ctr[CTR_NEGMIN] ? (1 << 30) - ctr[CTR_NEGMIN] : 0;
     if (err) {
         char buf[220];
@@ -430,6 +433,7 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     c->yee_index64 = false;
     c->dirty = false;
     c->max_known = c->min_known = 0;
+    c->n_dense = c->n_sparse = 0;
     c->force_class = -1;
     c->fixed_point = true;
     c->tmap_ok = false;
@@ -610,9 +614,14 @@ static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
         }
         // which variants to launch: a belief from the last synchronisation, with a margin; a supercell that crossed
         // the line since is still stepped correctly, by the variant that takes every supercell
+        // (the variant that "takes every supercell" steps one of the other class correctly, only slower: a class is
+        // dropped when it holds less than 1/64 of the non-empty supercells — a laser pulse that bunches a few hundred
+        // of 200 000 sparse supercells past the line must not switch the whole step to the mixed mode)
         d.class_all = 0;
-        if (c->max_known > 0 && c->max_known <= c->d.direct_below * 3 / 4) d.class_all = 1;
-        else if (c->min_known >= c->d.direct_below * 5 / 4) d.class_all = 2;
+        if (c->n_dense + c->n_sparse > 0) {
+            if ((long long)c->n_dense * 64 <= c->n_sparse) d.class_all = 1;
+            else if ((long long)c->n_sparse * 64 <= c->n_dense) d.class_all = 2;
+        }
         if (c->force_class >= 0) d.class_all = c->force_class;
         // A step that only launches the sparse variant accumulates J in float (shared tile and global array): its
         // supercells see few same-node collisions, and the 64-bit accumulators cost a memset and a convert pass over

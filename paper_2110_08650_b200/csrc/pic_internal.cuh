@@ -38,6 +38,8 @@ enum {
     CTR_OVF = 7,
     CTR_FREE_TOP = 8,     // entries on the stack of returned frames (may dip below 0 while prepare pops)          // entries in the overflow queue of out-of-window particles (this step)
        // bits of max |weight| loaded so far (non-negative floats order like ints)
+    CTR_NDENSE = 12,      // non-empty supercells at or above the sparse/dense line after this step (pic_prepare_kernel)
+    CTR_NSPARSE = 13,     // non-empty supercells below it
     CTR_CROWD = 11,       // entries in crowd_list (supercells the next step starts first), built by pic_prepare_kernel
     CTR_WORK = 10,        // next supercell of the persistent step kernel (zeroed before every launch)
     CTR_NEGMIN = 9,       // max over non-empty supercells of (2^30 - population) seen by pic_prepare_kernel, i.e. 2^30 - min

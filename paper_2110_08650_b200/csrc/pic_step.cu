@@ -710,6 +710,17 @@ __global__ void pic_prepare_kernel(const PicDev d)
     // (largest population seen: particles, not slots — after a step without a sort `count` includes the holes)
     atomicMax(d.ctr + CTR_MAX_COUNT, (d.nosort ? next : count + inc));
     if (next > 0) atomicMax(d.ctr + CTR_NEGMIN, (1 << 30) - next);
+    // how many supercells fall on either side of the sparse/dense line (one atomic per warp and side): the host reads
+    // the two counts at its next synchronisation and launches one class of variants only where the other is < 2 %
+    {
+        const unsigned m = __activemask();              // (threads beyond the last supercell or after a fault have left)
+        const unsigned dense = __ballot_sync(m, next >= d.direct_below);
+        const unsigned sparse = __ballot_sync(m, next > 0 && next < d.direct_below);
+        if ((int)(threadIdx.x & 31) == __ffs(m) - 1) {
+            if (dense) atomicAdd(d.ctr + CTR_NDENSE, __popc(dense));
+            if (sparse) atomicAdd(d.ctr + CTR_NSPARSE, __popc(sparse));
+        }
+    }
 }
 
 // Table regions abandoned by the pic_prepare_kernel launched just before go back to the free list of their class
@@ -995,7 +1006,7 @@ cudaError_t pic_launch_convert(const PicDev& d, cudaStream_t st, int64_t* launch
 
 cudaError_t pic_launch_prepare(const PicDev& d, cudaStream_t st, int64_t* launches)
 {
-    cudaError_t e0 = cudaMemsetAsync(d.ctr + CTR_CROWD, 0, sizeof(int), st);      // the list is rebuilt by every prepare
+    cudaError_t e0 = cudaMemsetAsync(d.ctr + CTR_CROWD, 0, 3 * sizeof(int), st);  // crowd list and the two class counts (CTR_CROWD, CTR_NDENSE, CTR_NSPARSE are adjacent) are rebuilt by every prepare
     if (e0 != cudaSuccess) return e0;
     pic_prepare_kernel<<<(d.nsc + 255) / 256, 256, 0, st>>>(d);
     pic_reclaim_tables_kernel<<<(d.nsc + 255) / 256, 256, 0, st>>>(d);
