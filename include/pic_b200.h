@@ -214,6 +214,12 @@ const char* pic_last_error(const pic_ctx* ctx);   /* ctx may be NULL: last creat
 
 int32_t pic_destroy(pic_ctx* ctx);                /* frees host state only */
 
+/* Replace the current the next pic_update_fields uses (device pointers, layout of pic_get_current; device-to-device
+ * copies on the stream).  For a domain decomposition above this library: a rank's own deposit lacks what
+ * its neighbours deposited into its boundary cells; after the guard-plane exchange the completed J is put back here
+ * before the field update.  The next pic_step overwrites it. */
+int32_t pic_set_current(pic_ctx* ctx, const float* Jx, const float* Jy, const float* Jz);
+
 /* ONE entry point that allocates nothing and needs no context or workspace, for callers that cannot call cudaMalloc
  * (code under CUDA graph capture, tight serving loops, harnesses that forbid allocation): the Esirkepov deposit
  * (the same arithmetic as the step's per-particle deposit) of n particles given their positions

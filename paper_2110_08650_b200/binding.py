@@ -23,7 +23,7 @@ SYMBOLS = (
     "pic_workspace_bytes", "pic_create", "pic_set_species", "pic_load_particles", "pic_set_fields",
     "pic_step", "pic_get_current", "pic_get_particles", "pic_get_counts", "pic_get_stats", "pic_sync",
     "pic_set_option", "pic_get_timing", "pic_launch_count", "pic_last_error", "pic_destroy",
-    "pic_update_fields", "pic_get_fields", "pic_deposit_current_noalloc",
+    "pic_update_fields", "pic_get_fields", "pic_deposit_current_noalloc", "pic_set_current",
 )
 
 
@@ -184,6 +184,14 @@ class Pic:
         nb = self.n_cells * 4
         self._check(self._L.pic_get_fields(self._h, *[C.c_void_p(F.data_ptr() + c * nb) for c in range(6)]))
         return F
+
+    def set_current(self, J: torch.Tensor):
+        """J: float32 [3, nz, ny, nx] on the device: the current the next update_fields uses (pic_set_current)."""
+        nx, ny, nz = self.grid
+        if tuple(J.shape) != (3, nz, ny, nx) or J.dtype != torch.float32 or not J.is_cuda or not J.is_contiguous():
+            raise ValueError("J: expected a contiguous CUDA float32 tensor of shape [3, nz, ny, nx]")
+        nb = self.n_cells * 4
+        self._check(self._L.pic_set_current(self._h, *[C.c_void_p(J.data_ptr() + c * nb) for c in range(3)]))
 
     def get_current(self) -> torch.Tensor:
         """float32 [3, nz, ny, nx]: J of the last step."""

@@ -734,6 +734,19 @@ int32_t pic_get_current(pic_ctx* c, float* Jx, float* Jy, float* Jz)
     return PIC_OK;
 }
 
+int32_t pic_set_current(pic_ctx* c, const float* Jx, const float* Jy, const float* Jz)
+{
+    if (!c) return PIC_EINVAL;
+    const float* src[3] = {Jx, Jy, Jz};
+    const size_t ncell = (size_t)c->d.nx * c->d.ny * c->d.nz;
+    for (int k = 0; k < 3; ++k) {
+        if (!src[k]) return fail(c, PIC_EINVAL, "pic_set_current: NULL component");
+        cudaError_t e = cudaMemcpyAsync(c->d.J + k * ncell, src[k], ncell * sizeof(float), cudaMemcpyDeviceToDevice, c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e, "pic_set_current: cudaMemcpyAsync");
+    }
+    return PIC_OK;
+}
+
 int32_t pic_get_particles(pic_ctx* c, int64_t capacity, int64_t* n_out, double* x, double* y, double* z,
                           float* ux, float* uy, float* uz, float* w, int32_t* species, uint32_t* id,
                           int32_t* supercell)

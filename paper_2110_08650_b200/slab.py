@@ -16,8 +16,9 @@ This module is the host logic: ownership, packing, the neighbour exchange over `
 calls (NCCL on GPUs, gloo in the CPU tests) or, for several ranks emulated in ONE process, a loop-back exchange —
 and `SlabRank`, which drives a local stepper (the CUDA library through `binding.Pic`, or any object with the same five
 calls).  It holds none of the method's arithmetic.  State of the art here: correct by construction and tested at
-world size 2 with gloo and, on one GPU, as two emulated ranks against the single-domain run; no multi-GPU hardware was
-available to time it, and `bench.py --gpus N` still runs replicas.
+world size 2 with gloo and, on one GPU, as emulated ranks against the single-domain run — static fields and the
+self-consistent loop with the E/B halo exchange; no multi-GPU hardware was available to time it, and
+`bench.py --gpus N` still runs replicas.
 """
 from __future__ import annotations
 
@@ -215,6 +216,16 @@ class PicStepper:
             return torch.zeros((3, g[2], g[1], g[0]), dtype=torch.float32, device=self.device)
         return self.pic.get_current()
 
+    # ---- evolving fields: the completed J goes back in before the Yee update (pic_set_current)
+    def set_current(self, J: torch.Tensor):
+        self.pic.set_current(J.to(self.device, torch.float32).contiguous())
+
+    def update_fields(self):
+        self.pic.update_fields()
+
+    def fields(self) -> torch.Tensor:
+        return self.pic.get_fields()
+
 
 class SlabRank:
     """One rank's share of the domain: its particles (global coordinates, global ids) and its owned planes of J."""
@@ -251,6 +262,7 @@ class SlabRank:
         self.parts["z"] = dec.to_global_z(self.rank, P["z"])
         self.parts["gid"] = gid
         self._J_local = st.current()
+        self._st = st
 
     def outgoing_particles(self) -> Tuple[torch.Tensor, torch.Tensor]:
         dec = self.dec
@@ -281,8 +293,23 @@ class SlabRank:
         self.J[:, own - G:] += from_hi.permute(1, 0, 2, 3).to(self.J.device)
 
 
-def slab_step(ranks: List[SlabRank], exchange) -> None:
-    """One step of every rank in `ranks` (one entry with DistExchange, all ranks with LoopbackExchange)."""
+def _owned_edge_planes(A: torch.Tensor, dec: SlabDecomposition) -> Tuple[torch.Tensor, torch.Tensor]:
+    """A: [C, owned, ny, nx] -> (bottom G planes for the lower neighbour, top G planes for the upper one), planes first."""
+    G = dec.guard
+    return A[:, :G].permute(1, 0, 2, 3).contiguous(), A[:, -G:].permute(1, 0, 2, 3).contiguous()
+
+
+def _with_guards(A: torch.Tensor, from_lo: torch.Tensor, from_hi: torch.Tensor) -> torch.Tensor:
+    """Owned planes + the neighbours' edge planes as guards: [C, G + owned + G, ny, nx]."""
+    return torch.cat([from_lo.permute(1, 0, 2, 3).to(A.device, A.dtype), A, from_hi.permute(1, 0, 2, 3).to(A.device, A.dtype)], 1).contiguous()
+
+
+def slab_step(ranks: List[SlabRank], exchange, evolve_fields: bool = False) -> None:
+    """One step of every rank in `ranks` (one entry with DistExchange, all ranks with LoopbackExchange).
+    evolve_fields: the step ends with the Yee update of E, B on every slab: the completed J is
+    extended by the neighbours' edge planes (the update of an owned cell reads J, E, B up to two cells away: less than
+    the guard), the local update runs on slab + guards, and the guards of the new E, B are refreshed from the
+    neighbours' owned planes — the E/B halo exchange."""
     for r in ranks:
         r.local_step()
     inc = exchange.swap_all([r.outgoing_particles() for r in ranks])
@@ -291,3 +318,15 @@ def slab_step(ranks: List[SlabRank], exchange) -> None:
     inc = exchange.swap_all([r.outgoing_current() for r in ranks])
     for r, (flo, fhi) in zip(ranks, inc):
         r.incoming_current(flo, fhi)
+    if not evolve_fields:
+        return
+    dec = ranks[0].dec
+    G, own = dec.guard, dec.owned_cells
+    inc = exchange.swap_all([_owned_edge_planes(r.J, dec) for r in ranks])
+    for r, (flo, fhi) in zip(ranks, inc):
+        r._st.set_current(_with_guards(r.J, flo, fhi))
+        r._st.update_fields()
+        r._F_owned = r._st.fields()[:, G:G + own].clone()
+    inc = exchange.swap_all([_owned_edge_planes(r._F_owned, dec) for r in ranks])
+    for r, (flo, fhi) in zip(ranks, inc):
+        r.fields_local = _with_guards(r._F_owned, flo, fhi)

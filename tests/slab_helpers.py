@@ -37,6 +37,15 @@ class OracleStepper:
     def current(self):
         return torch.from_numpy(np.stack(self.orc.J))
 
+    def set_current(self, J):
+        self.orc.J = tuple(np.ascontiguousarray(j, dtype=np.float64) for j in J.numpy())
+
+    def update_fields(self):
+        self.orc.update_fields()
+
+    def fields(self):
+        return torch.from_numpy(np.stack(self.orc.fields))
+
 
 def global_particles(parts):
     """workloads.ParticleChunk -> dict with global ids."""

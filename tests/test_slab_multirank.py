@@ -125,3 +125,87 @@ def test_two_processes_over_gloo():
     dec = SL.SlabDecomposition(wl.grid, wl.cell, wl.supercell, world)
     state = [(r, {k: torch.from_numpy(v) for k, v in res[r][0].items()}, torch.from_numpy(res[r][1])) for r in range(world)]
     _check(wl, dec, state, ref_P, ref_J)
+
+
+def _loop_case(order=2, grid=(16, 16, 32)):
+    # a weakly coupled plasma (omega_p dt = 0.14) with fast particles: the fields visibly change and particles cross slabs
+    wl = W.CONFIGS["thermal_128"].scaled(grid, shape_order=order, ppc=2, u_th=0.3)
+    parts, fields = W.make_particles(wl), W.make_fields(wl)
+    parts.w.mul_(0.04)
+    return wl, parts, fields
+
+
+def _single_domain_loop(wl, parts, fields, n_steps):
+    import oracle
+    orc = oracle.Oracle(wl.grid, wl.cell, wl.dt, wl.supercell, wl.shape_order)
+    orc.load_particles(*(getattr(parts, k).numpy() for k in ("x", "y", "z", "ux", "uy", "uz", "w")),
+                       species=parts.species.numpy())
+    orc.set_fields(fields.numpy())
+    assert orc.step(n_steps, update_fields=True) == 0
+    return orc.particles(), np.stack(orc.J), np.stack(orc.fields)
+
+
+def _check_fields(dec, ranks_fields, ref_F, ref_F0):
+    scale = np.abs(ref_F).max()
+    assert np.abs(ref_F - ref_F0).max() > 0.02 * scale, "the fields must have changed: this is not the static-field path"
+    for rank, F in ranks_fields:
+        z0, z1 = dec.z_range(rank)
+        G = dec.guard
+        assert np.abs(F[:, G:G + dec.owned_cells] - ref_F[:, z0:z1]).max() <= 1e-12 * scale
+        # and the refreshed guards are the neighbours' planes
+        idx = np.arange(z0 - G, z1 + G) % dec.grid[2]
+        assert np.abs(F - ref_F[:, idx]).max() <= 1e-12 * scale
+
+
+@pytest.mark.parametrize("world", (1, 2, 4))
+def test_loopback_ranks_self_consistent_loop(world):
+    """With the Yee update on every slab: J extended by the neighbours' edge planes, local update on slab + guards,
+    E/B halo exchange.  Particles, J and fields against the single-domain self-consistent oracle."""
+    from slab_helpers import OracleStepper, global_particles
+    wl, parts, fields = _loop_case()
+    n_steps = 4
+    ref_P, ref_J, ref_F = _single_domain_loop(wl, parts, fields, n_steps)
+    dec = SL.SlabDecomposition(wl.grid, wl.cell, wl.supercell, world)
+    make = lambda g: OracleStepper(g, wl.cell, wl.dt, wl.supercell, wl.shape_order)
+    ranks = [SL.SlabRank(dec, r, make, real=torch.float64) for r in range(world)]
+    gp = global_particles(parts)
+    for r in ranks:
+        r.take_owned(gp)
+        r.set_global_fields(fields.to(torch.float64))
+    ex = SL.LoopbackExchange(dec)
+    for _ in range(n_steps):
+        SL.slab_step(ranks, ex, evolve_fields=True)
+    _check(wl, dec, [(r.rank, r.parts, r.J) for r in ranks], ref_P, ref_J)
+    _check_fields(dec, [(r.rank, r.fields_local.numpy()) for r in ranks], ref_F, fields.numpy().astype(np.float64))
+
+
+def _worker_loop(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from slab_helpers import OracleStepper, global_particles
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    wl, parts, fields = _loop_case()
+    dec = SL.SlabDecomposition(wl.grid, wl.cell, wl.supercell, world)
+    me = SL.SlabRank(dec, rank, lambda g: OracleStepper(g, wl.cell, wl.dt, wl.supercell, wl.shape_order), real=torch.float64)
+    me.take_owned(global_particles(parts))
+    me.set_global_fields(fields.to(torch.float64))
+    ex = SL.DistExchange(dec, rank)
+    for _ in range(4):
+        SL.slab_step([me], ex, evolve_fields=True)
+    dist.barrier()
+    out[rank] = ({k: v.numpy() for k, v in me.parts.items()}, me.J.numpy(), me.fields_local.numpy())
+    dist.destroy_process_group()
+
+
+def test_two_processes_over_gloo_self_consistent_loop():
+    world = 2
+    wl, parts, fields = _loop_case()
+    ref_P, ref_J, ref_F = _single_domain_loop(wl, parts, fields, 4)
+    with mp.Manager() as m:
+        out = m.dict()
+        mp.spawn(_worker_loop, args=(world, 29549, out), nprocs=world, join=True)
+        res = dict(out)
+    dec = SL.SlabDecomposition(wl.grid, wl.cell, wl.supercell, world)
+    state = [(r, {k: torch.from_numpy(v) for k, v in res[r][0].items()}, torch.from_numpy(res[r][1])) for r in range(world)]
+    _check(wl, dec, state, ref_P, ref_J)
+    _check_fields(dec, [(r, res[r][2]) for r in range(world)], ref_F, fields.numpy().astype(np.float64))
