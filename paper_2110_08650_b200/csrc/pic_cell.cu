@@ -815,7 +815,7 @@ static cudaError_t launch_cell_one(const PicDev& d, const CUtensorMap& map, cuda
         if (ctas < 2) return cudaErrorLaunchOutOfResources;
         configured = true;
     }
-    pic_cell_kernel<O, TMA><<<d.nsc + PIC_CROWD_MAX, PIC_CELL_THREADS, bytes, st>>>(d, map);
+    pic_cell_kernel<O, TMA><<<pic_step_grid(d), PIC_CELL_THREADS, bytes, st>>>(d, map);
     return cudaGetLastError();
 }
 

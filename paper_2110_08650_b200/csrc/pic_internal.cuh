@@ -154,10 +154,14 @@ __host__ __device__ inline int pic_segment_target(int supercell_count, int seg_n
 // Returns -1 for a CTA without work.
 __device__ inline int pic_cta_supercell(const PicDev& d, int block)
 {
+    if (d.crowd_min >= (1 << 30)) return block;      // option crowd_first off (default): the grid has no extra CTAs
     if (block < PIC_CROWD_MAX) return block < d.ctr[CTR_CROWD] ? d.crowd_list[block] : -1;
     const int s = block - PIC_CROWD_MAX;
     return d.sc_crowd[s] ? -1 : s;
 }
+
+// CTAs of a step-kernel launch (see pic_cta_supercell)
+inline int pic_step_grid(const PicDev& d) { return d.nsc + (d.crowd_min >= (1 << 30) ? 0 : PIC_CROWD_MAX); }
 
 __host__ __device__ inline uint32_t pic_pack_bits(int local_cell, int species)
 {

@@ -915,7 +915,7 @@ static cudaError_t launch_step_one(const PicDev& d, const CUtensorMap& map, cuda
         if (ctas < 2) return cudaErrorLaunchOutOfResources;
         configured = true;
     }
-    pic_step_kernel<O, TMA, FIX, MODE><<<d.nsc + PIC_CROWD_MAX, SPARSE ? 256 : PIC_STEP_THREADS, bytes, st>>>(d, map);
+    pic_step_kernel<O, TMA, FIX, MODE><<<pic_step_grid(d), SPARSE ? 256 : PIC_STEP_THREADS, bytes, st>>>(d, map);
     return cudaGetLastError();
 }
 
