@@ -26,7 +26,7 @@ struct pic_ctx {
     int cell_kernel;             // option "cell_kernel": dense supercells go to 0 the round-1 kernels, 1 pic_cell_kernel, 2 the persistent pic_pcell_kernel
     bool fuse_sort;              // option "fuse_sort": the step kernel sorts its supercell first (default on)
     bool field_update;           // option "field_update": every step ends with a Yee update of E, B (pic_fields.cu)
-    float* Fbuf[2];              // the two plain field buffers; d.F == Fbuf[F_cur]
+    float* Fbuf[2];              // the two PADDED field buffers (periodic halos pre-filled); d.Fpad == Fbuf[F_cur]
     int F_cur;
     bool yee_index64;            // option "yee_index64": force the 64-bit-index instantiation (taken anyway beyond 2^32 elements)
     int yee_tile;                // option "yee_tile": y extent of the Yee kernel's tile (8 or 16)
@@ -44,7 +44,7 @@ struct pic_ctx {
     uint64_t ws_bytes;
     std::string err;
     // TMA descriptor of the padded field copy
-    alignas(64) unsigned char tmap[128];
+    alignas(64) unsigned char tmap[2][128];     // one tensor map per padded buffer
     bool tmap_ok;
     // option "timing": CUDA events around every launch of the step kernel
     bool timing;
@@ -60,7 +60,7 @@ namespace {
 
 struct Layout {
     uint64_t rec0, rec1, pid0, pid1, free_stack, tbl_pool, tbl_off, tbl_cap, tbl_old_off, tbl_old_cap, tbl_free, tbl_free_top, sc_nframes, sc_count, sc_tail, sc_incoming,
-        sc_left, sc_next, sc_crowd, crowd_list, cell_off, cell_hist, cell_perm, cell_kbase, x_rec, x_id, x_dst, ovf, ctr, ctr64, F, F2, Fpad, J, J64, sc_offset, total;
+        sc_left, sc_next, sc_crowd, crowd_list, cell_off, cell_hist, cell_perm, cell_kbase, x_rec, x_id, x_dst, ovf, ctr, ctr64, Fpad, Fpad2, J, J64, sc_offset, total;
     int n_frames, tbl_pool_size, x_cap, nsc;
 };
 
@@ -115,9 +115,11 @@ int compute_layout(const int32_t grid[3], const int32_t sc[3], int order, int64_
     L->ovf = take(xcap * 32);
     L->ctr = take(CTR_N * 4);
     L->ctr64 = take(CTR64_N * 8);
-    L->F = take(6 * ncell * 4);
-    L->F2 = take(6 * ncell * 4);                 // second field buffer of the Yee update (pic_fields.cu)
-    L->Fpad = take(6ull * (grid[0] + PIC_PAD_X) * (grid[1] + PIC_PAD_Y) * (grid[2] + PIC_PAD_Z) * 4);
+    // the fields live in PADDED arrays only (what the step kernel's TMA reads); two of them: the Yee update reads level
+    // n from one and writes level n+1, every periodic image included, to the other
+    const uint64_t npad6 = 6ull * (grid[0] + PIC_PAD_X) * (grid[1] + PIC_PAD_Y) * (grid[2] + PIC_PAD_Z) * 4;
+    L->Fpad = take(npad6);
+    L->Fpad2 = take(npad6);
     L->J = take(3 * ncell * 4);
     L->J64 = take(3 * ncell * 8);
     L->sc_offset = take((nsc + 1) * 8);
@@ -286,12 +288,13 @@ __global__ void pic_get_particles_kernel(const PicDev d, const GetArgs a)
     }
 }
 
-// Padded copy of the fields with periodic halos (source of the TMA tile loads).
-__global__ void pic_pad_fields_kernel(const PicDev d, float* dst)
+// Caller's plain arrays -> padded array with periodic halos (the only form the fields are kept in), and back.
+struct FieldPtrs { const float* src[6]; float* dst[6]; };
+
+__global__ void pic_pad_fields_kernel(const PicDev d, const FieldPtrs f, float* pad)
 {
     const int px = d.nx + PIC_PAD_X, py = d.ny + PIC_PAD_Y, pz = d.nz + PIC_PAD_Z;
     const size_t n = (size_t)6 * px * py * pz;
-    const size_t ncell = (size_t)d.nx * d.ny * d.nz;
     for (size_t e = blockIdx.x * (size_t)blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
         size_t r = e;
         int i = (int)(r % px); r /= px;
@@ -301,7 +304,23 @@ __global__ void pic_pad_fields_kernel(const PicDev d, float* dst)
         int gi = ((i - d.pad_lo_x) % d.nx + d.nx) % d.nx;
         int gj = ((j - PIC_PAD_LO) % d.ny + d.ny) % d.ny;
         int gk = ((k - PIC_PAD_LO) % d.nz + d.nz) % d.nz;
-        dst[e] = d.F[c * ncell + (size_t)gi + (size_t)d.nx * ((size_t)gj + (size_t)d.ny * gk)];
+        pad[e] = f.src[c][(size_t)gi + (size_t)d.nx * ((size_t)gj + (size_t)d.ny * gk)];
+    }
+}
+
+__global__ void pic_unpad_fields_kernel(const PicDev d, const FieldPtrs f, const float* pad)
+{
+    const int px = d.nx + PIC_PAD_X, py = d.ny + PIC_PAD_Y, pz = d.nz + PIC_PAD_Z;
+    const size_t ncell = (size_t)d.nx * d.ny * d.nz;
+    for (size_t e = blockIdx.x * (size_t)blockDim.x + threadIdx.x; e < 6 * ncell; e += (size_t)gridDim.x * blockDim.x) {
+        const int c = (int)(e / ncell);
+        if (!f.dst[c]) continue;
+        size_t r = e % ncell;
+        const int i = (int)(r % d.nx); r /= d.nx;
+        const int j = (int)(r % d.ny);
+        const int k = (int)(r / d.ny);
+        f.dst[c][e - c * ncell] = pad[(size_t)c * px * py * pz + (size_t)(i + d.pad_lo_x) +
+                                      (size_t)px * ((size_t)(j + PIC_PAD_LO) + (size_t)py * (k + PIC_PAD_LO))];
     }
 }
 
@@ -352,7 +371,7 @@ int check_device(pic_ctx* c)
 // 4-D tensor map (x, y, z, component) over the padded field copy; the step kernel
 // fetches a supercell's whole E/B tile with one cp.async.bulk.tensor.
 // cuTensorMapEncodeTiled is resolved through the runtime, so libcuda is not a link dependency.
-static int pic_build_tensor_map(pic_ctx* c)
+static int pic_build_tensor_map(pic_ctx* c, int which)
 {
     typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -372,7 +391,7 @@ static int pic_build_tensor_map(pic_ctx* c)
     const cuuint64_t strides[3] = {px * 4, px * py * 4, px * py * pz * 4};
     const cuuint32_t box[4] = {12, fn_xy, fn_xy - (PIC_SCX - PIC_SCZ), 6};
     const cuuint32_t estr[4] = {1, 1, 1, 1};
-    CUresult r = ((encode_fn)fn)((CUtensorMap*)c->tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void*)d.Fpad, dims,
+    CUresult r = ((encode_fn)fn)((CUtensorMap*)c->tmap[which], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void*)c->Fbuf[which], dims,
                                  strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                  CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(c, PIC_ECUDA, "cuTensorMapEncodeTiled failed");
@@ -491,14 +510,14 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     d.ovf = (float4*)(w + L.ovf); d.ovf_cap = L.x_cap;
     d.x_id = (uint32_t*)(w + L.x_id); d.x_dst = (int*)(w + L.x_dst); d.x_cap = L.x_cap;
     d.ctr = (int*)(w + L.ctr); d.ctr64 = (unsigned long long*)(w + L.ctr64);
-    c->Fbuf[0] = (float*)(w + L.F); c->Fbuf[1] = (float*)(w + L.F2); c->F_cur = 0;
-    d.F = (const float*)(w + L.F); d.Fpad = (const float*)(w + L.Fpad); d.J = (float*)(w + L.J); d.J64 = (long long*)(w + L.J64);
+    c->Fbuf[0] = (float*)(w + L.Fpad); c->Fbuf[1] = (float*)(w + L.Fpad2); c->F_cur = 0;
+    d.Fpad = c->Fbuf[0]; d.J = (float*)(w + L.J); d.J64 = (long long*)(w + L.J64);
     d.sc_offset = (long long*)(w + L.sc_offset);
     d.pad_lo_x = (shape_order == 3) ? 2 : 1;
 
     // zero the bookkeeping region [tbl_off, x_rec) and the counters, J
     cudaError_t e = cudaMemsetAsync(w + L.tbl_off, 0, L.x_rec - L.tbl_off, c->stream);
-    if (e == cudaSuccess) e = cudaMemsetAsync(w + L.ctr, 0, L.F - L.ctr, c->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(w + L.ctr, 0, L.Fpad - L.ctr, c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(w + L.J, 0, L.sc_offset - L.J, c->stream);
     if (e != cudaSuccess) { int r = cuda_fail(nullptr, e, "pic_create: cudaMemsetAsync"); delete c; return r; }
     *out = c;
@@ -559,19 +578,14 @@ int32_t pic_set_fields(pic_ctx* c, const float* Ex, const float* Ey, const float
                        const float* Bx, const float* By, const float* Bz)
 {
     if (!c) return PIC_EINVAL;
-    const float* src[6] = {Ex, Ey, Ez, Bx, By, Bz};
-    const size_t ncell = (size_t)c->d.nx * c->d.ny * c->d.nz;
-    for (int k = 0; k < 6; ++k) {
-        if (!src[k]) return fail(c, PIC_EINVAL, "pic_set_fields: NULL component");
-        cudaError_t e = cudaMemcpyAsync((float*)c->d.F + k * ncell, src[k], ncell * sizeof(float),
-                                        cudaMemcpyDeviceToDevice, c->stream);
-        if (e != cudaSuccess) return cuda_fail(c, e, "pic_set_fields: cudaMemcpyAsync");
-    }
-    pic_pad_fields_kernel<<<148 * 8, 256, 0, c->stream>>>(c->d, (float*)c->d.Fpad);
+    FieldPtrs f = {{Ex, Ey, Ez, Bx, By, Bz}, {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr}};
+    for (int k = 0; k < 6; ++k)
+        if (!f.src[k]) return fail(c, PIC_EINVAL, "pic_set_fields: NULL component");
+    pic_pad_fields_kernel<<<148 * 8, 256, 0, c->stream>>>(c->d, f, c->Fbuf[c->F_cur]);
     c->launches += 1;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(c, e, "pic_set_fields: pad kernel");
-    if (!c->tmap_ok) c->tmap_ok = (pic_build_tensor_map(c) == PIC_OK);
+    if (!c->tmap_ok) c->tmap_ok = (pic_build_tensor_map(c, 0) == PIC_OK && pic_build_tensor_map(c, 1) == PIC_OK);
     c->have_fields = true;
     return PIC_OK;
 }
@@ -590,13 +604,13 @@ static int ensure_sorted(pic_ctx* c)
     return PIC_OK;
 }
 
-// One Yee update with the last step's J: level n in Fbuf[F_cur] -> level n+1 in the other buffer and in Fpad.
+// One Yee update with the last step's J: level n in the padded buffer Fbuf[F_cur] -> level n+1 in the other one.
 static cudaError_t enqueue_field_update(pic_ctx* c, cudaStream_t st)
 {
     cudaError_t e = pic_launch_yee(c->d, c->Fbuf[c->F_cur], c->Fbuf[c->F_cur ^ 1], c->dt, c->cell, c->yee_tile, c->yee_index64, st, &c->launches);
     if (e != cudaSuccess) return e;
     c->F_cur ^= 1;
-    c->d.F = c->Fbuf[c->F_cur];
+    c->d.Fpad = c->Fbuf[c->F_cur];
     return cudaSuccess;
 }
 
@@ -665,7 +679,7 @@ static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
             ds.sort_filter = d.class_all == 1 ? 0 : 1;
             if (e == cudaSuccess) e = pic_launch_sort(ds, st, &c->launches);
         }
-        if (e == cudaSuccess) e = pic_launch_step(d, c->order, c->use_tma && c->tmap_ok, fix, c->tmap, st, &c->launches, c->cell_kernel);
+        if (e == cudaSuccess) e = pic_launch_step(d, c->order, c->use_tma && c->tmap_ok, fix, c->tmap[c->F_cur], st, &c->launches, c->cell_kernel);
         d.fused = 0;
         if (e == cudaSuccess && c->timing) {
             e = cudaEventRecord(ev1, st);
@@ -709,14 +723,11 @@ int32_t pic_get_fields(pic_ctx* c, float* Ex, float* Ey, float* Ez, float* Bx, f
 {
     if (!c) return PIC_EINVAL;
     if (!c->have_fields) return fail(c, PIC_ESTATE, "pic_get_fields: pic_set_fields has not been called");
-    float* dst[6] = {Ex, Ey, Ez, Bx, By, Bz};
-    const size_t ncell = (size_t)c->d.nx * c->d.ny * c->d.nz;
-    for (int k = 0; k < 6; ++k) {
-        if (!dst[k]) continue;
-        cudaError_t e = cudaMemcpyAsync(dst[k], c->d.F + k * ncell, ncell * sizeof(float),
-                                        cudaMemcpyDeviceToDevice, c->stream);
-        if (e != cudaSuccess) return cuda_fail(c, e, "pic_get_fields: cudaMemcpyAsync");
-    }
+    FieldPtrs f = {{nullptr, nullptr, nullptr, nullptr, nullptr, nullptr}, {Ex, Ey, Ez, Bx, By, Bz}};
+    pic_unpad_fields_kernel<<<148 * 8, 256, 0, c->stream>>>(c->d, f, c->Fbuf[c->F_cur]);
+    c->launches += 1;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e, "pic_get_fields: unpad kernel");
     return PIC_OK;
 }
 

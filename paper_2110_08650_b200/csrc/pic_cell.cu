@@ -254,7 +254,6 @@ __device__ __forceinline__ int cell_prologue(const PicDev& d, const CUtensorMap*
                         oz + PIC_PAD_LO - G::FL, 0);
         }
     } else {
-        const size_t ncell = (size_t)d.nx * d.ny * d.nz;
         for (int e = tid; e < 6 * G::FNZ * G::FNY * G::FNX; e += NT) {
             int i = e % G::FNX;
             int r = e / G::FNX;
@@ -265,7 +264,7 @@ __device__ __forceinline__ int cell_prologue(const PicDev& d, const CUtensorMap*
             int gi = wrapi(ox + i - G::FL, d.nx), gj = wrapi(oy + j - G::FL, d.ny),
                 gk = wrapi(oz + k - G::FL, d.nz);
             v.sF[c * G::FCOMP + (k * G::FNY + j) * G::FPX + i] =
-                __ldg(d.F + c * ncell + (size_t)gi + (size_t)d.nx * ((size_t)gj + (size_t)d.ny * gk));
+                __ldg(d.Fpad + pic_padded_index(d, c, gi, gj, gk));
         }
     }
     // scratch of the fused sort and of the cell order: the leaver staging area, unused until the particle loop

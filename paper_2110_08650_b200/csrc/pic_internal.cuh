@@ -113,8 +113,8 @@ struct PicDev {
     int* ctr;
     unsigned long long* ctr64;
     // grids
-    const float* F;              // 6 components x ncell (Ex,Ey,Ez,Bx,By,Bz), unpadded
-    const float* Fpad;           // padded copy for TMA: [6][nz+PZ][ny+PY][nx+PX]
+    const float* Fpad;           // the fields (Ex,Ey,Ez,Bx,By,Bz), kept padded with periodic halos only — what the TMA
+                                 // tile loads read: [6][nz+PZ][ny+PY][nx+PX]; node (i,j,k) at pic_padded_index()
     int pad_lo_x;                // x halo below node 0 in Fpad = the tile's guard width, so that
                                  // every TMA box starts on a 16-byte boundary
     float* J;                    // 3 components x ncell
@@ -123,11 +123,18 @@ struct PicDev {
     long long* sc_offset;        // [nsc+1] exclusive scan of sc_count (pic_get_particles)
 };
 
-// padding of the TMA copy of the fields (periodic halos pre-filled)
+// padding of the field arrays (periodic halos pre-filled)
 #define PIC_PAD_LO 2
 #define PIC_PAD_X 8              // nx + 8 keeps the row pitch a multiple of 16 bytes
 #define PIC_PAD_Y 4
 #define PIC_PAD_Z 4
+
+// element of component c at node (i,j,k), 0 <= i < nx etc., in the padded field array
+__host__ __device__ __forceinline__ size_t pic_padded_index(const PicDev& d, int c, int i, int j, int k)
+{
+    const size_t px = d.nx + PIC_PAD_X, py = d.ny + PIC_PAD_Y, pz = d.nz + PIC_PAD_Z;
+    return (size_t)(i + d.pad_lo_x) + px * ((size_t)(j + PIC_PAD_LO) + py * ((size_t)(k + PIC_PAD_LO) + pz * c));
+}
 
 // Work items of the step kernel: a cell of n particles is cut into ceil(n/T) segments, with T about
 // 3/4 of the supercell's mean cell population (measured optimum of balance vs. flushes).
@@ -180,6 +187,6 @@ cudaError_t pic_launch_zero_ints(int* p, size_t n, cudaStream_t st, int64_t* lau
 cudaError_t pic_launch_prepare(const PicDev& d, cudaStream_t st, int64_t* launches);
 cudaError_t pic_launch_scatter(const PicDev& d, cudaStream_t st, int64_t* launches);
 cudaError_t pic_launch_sort(const PicDev& d, cudaStream_t st, int64_t* launches);   // pool cur -> the other
-// pic_fields.cu: one Yee update F_in (level n) -> F_out (level n+1) and the padded copy d.Fpad, with J = d.J
+// pic_fields.cu: one Yee update, padded array F_in (level n) -> padded array F_out (level n+1, all periodic images), J = d.J
 cudaError_t pic_launch_yee(const PicDev& d, const float* F_in, float* F_out, double dt, const double cell[3], int tile_y,
                            bool index64, cudaStream_t st, int64_t* launches);

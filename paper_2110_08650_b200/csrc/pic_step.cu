@@ -111,7 +111,6 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
                         oz + PIC_PAD_LO - G::FL, 0);
         }
     } else {
-        const size_t ncell = (size_t)d.nx * d.ny * d.nz;
         for (int e = tid; e < 6 * G::FNZ * G::FNY * G::FNX; e += NT) {
             int i = e % G::FNX;
             int r = e / G::FNX;
@@ -122,7 +121,7 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
             int gi = wrapi(ox + i - G::FL, d.nx), gj = wrapi(oy + j - G::FL, d.ny),
                 gk = wrapi(oz + k - G::FL, d.nz);
             sF[c * G::FCOMP + (k * G::FNY + j) * G::FPX + i] =
-                __ldg(d.F + c * ncell + (size_t)gi + (size_t)d.nx * ((size_t)gj + (size_t)d.ny * gk));
+                __ldg(d.Fpad + pic_padded_index(d, c, gi, gj, gk));
         }
     }
     for (int e = tid; e < NJ; e += NT) sJhi[e] = 0;
