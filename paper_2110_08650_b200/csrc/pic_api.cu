@@ -30,6 +30,7 @@ struct pic_ctx {
     int F_cur;
     bool yee_index64;            // option "yee_index64": force the 64-bit-index instantiation (taken anyway beyond 2^32 elements)
     int yee_tile;                // option "yee_tile": y extent of the Yee kernel's tile (8 or 16)
+    bool yee_wide;               // option "yee_wide": four cells per thread where the grid is at least 64 wide (default)
     bool dirty;                  // pool cur holds a stepped state whose sort is still pending
     bool sparse_nosort;          // option "sparse_nosort": all-sparse steps skip the re-sort (default on)
     int steps_unsorted;          // steps since the last sort
@@ -449,6 +450,7 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     c->steps_unsorted = 0;
     c->field_update = false;
     c->yee_tile = 8;
+    c->yee_wide = true;
     c->yee_index64 = false;
     c->dirty = false;
     c->max_known = c->min_known = 0;
@@ -607,7 +609,7 @@ static int ensure_sorted(pic_ctx* c)
 // One Yee update with the last step's J: level n in the padded buffer Fbuf[F_cur] -> level n+1 in the other one.
 static cudaError_t enqueue_field_update(pic_ctx* c, cudaStream_t st)
 {
-    cudaError_t e = pic_launch_yee(c->d, c->Fbuf[c->F_cur], c->Fbuf[c->F_cur ^ 1], c->dt, c->cell, c->yee_tile, c->yee_index64, st, &c->launches);
+    cudaError_t e = pic_launch_yee(c->d, c->Fbuf[c->F_cur], c->Fbuf[c->F_cur ^ 1], c->dt, c->cell, c->yee_tile, c->yee_index64, c->yee_wide, st, &c->launches);
     if (e != cudaSuccess) return e;
     c->F_cur ^= 1;
     c->d.Fpad = c->Fbuf[c->F_cur];
@@ -869,6 +871,7 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
         return PIC_OK;
     }
     if (!strcmp(key, "yee_index64")) { c->yee_index64 = value != 0; return PIC_OK; }
+    if (!strcmp(key, "yee_wide")) { c->yee_wide = value != 0; return PIC_OK; }
     if (!strcmp(key, "yee_tile")) {
         if (value != 8 && value != 16) return fail(c, PIC_EINVAL, "pic_set_option: yee_tile must be 8 or 16");
         c->yee_tile = (int)value;

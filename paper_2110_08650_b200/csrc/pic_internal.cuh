@@ -189,4 +189,4 @@ cudaError_t pic_launch_scatter(const PicDev& d, cudaStream_t st, int64_t* launch
 cudaError_t pic_launch_sort(const PicDev& d, cudaStream_t st, int64_t* launches);   // pool cur -> the other
 // pic_fields.cu: one Yee update, padded array F_in (level n) -> padded array F_out (level n+1, all periodic images), J = d.J
 cudaError_t pic_launch_yee(const PicDev& d, const float* F_in, float* F_out, double dt, const double cell[3], int tile_y,
-                           bool index64, cudaStream_t st, int64_t* launches);
+                           bool index64, bool wide, cudaStream_t st, int64_t* launches);

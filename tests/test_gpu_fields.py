@@ -48,18 +48,47 @@ def test_vacuum_update_matches_oracle(grid, order, tile):
     pic.destroy()
 
 
+@pytest.mark.parametrize("grid", [(64, 16, 12), (72, 40, 80), (136, 24, 8), (40, 24, 20)])
+@pytest.mark.parametrize("order,tile,wide", ((2, 8, 1), (3, 8, 1), (2, 16, 1), (3, 16, 1), (2, 8, 0), (3, 16, 0)))
+def test_update_with_a_given_current_matches_oracle(grid, order, tile, wide):
+    """A random J set through set_current before every update: the J term and its indexing (unpadded, off the padded
+    arrays' 16-byte grid by pad_lo_x) in both field kernels — one cell per thread, and four per thread on grids at
+    least 64 wide (one tile, ragged second tile, two tiles and a rest; the last grid is too narrow and falls back)."""
+    wl, pic = _vacuum(grid, order)
+    pic.set_option("yee_tile", tile)
+    pic.set_option("yee_wide", wide)
+    F0 = W.make_fields(wl)
+    pic.set_fields(F0.cuda().contiguous())
+    F = [f.astype(np.float64) for f in F0.numpy()]
+    scale = max(np.abs(f).max() for f in F)
+    nx, ny, nz = grid
+    g = torch.Generator().manual_seed(nx * 7 + order)
+    for n in range(1, 5):
+        J = (torch.rand((3, nz, ny, nx), generator=g) - 0.5) * float(scale)
+        pic.set_current(J.cuda().contiguous())
+        pic.update_fields()
+        F = Y.yee_update(F, [j.astype(np.float64) for j in J.numpy()], wl.dt, wl.cell)
+        G = pic.get_fields().cpu().numpy().astype(np.float64)
+        err = np.abs(G - np.stack(F)).max()
+        assert err <= n * TOL_F * scale, (n, err / scale)
+    pic.sync()
+    pic.destroy()
+
+
 def test_index64_variant_matches_the_default_bit_for_bit():
-    """The 64-bit-index instantiation (taken by itself beyond 2^32 elements) on a small grid."""
-    out = []
-    for idx64 in (0, 1):
-        wl, pic = _vacuum((40, 24, 20), 3)
-        pic.set_option("yee_index64", idx64)
-        pic.set_fields(W.make_fields(wl).cuda().contiguous())
-        for _ in range(3):
-            pic.update_fields()
-        out.append(pic.get_fields().cpu())
-        pic.destroy()
-    assert torch.equal(out[0], out[1])
+    """The 64-bit-index instantiation (taken by itself beyond 2^32 elements) on a small grid and on one the
+    four-cell kernel takes."""
+    for grid in ((40, 24, 20), (72, 24, 20)):
+        out = []
+        for idx64 in (0, 1):
+            wl, pic = _vacuum(grid, 3)
+            pic.set_option("yee_index64", idx64)
+            pic.set_fields(W.make_fields(wl).cuda().contiguous())
+            for _ in range(3):
+                pic.update_fields()
+            out.append(pic.get_fields().cpu())
+            pic.destroy()
+        assert torch.equal(out[0], out[1])
 
 
 @pytest.mark.parametrize("name", ("lwfa", "pqs_large"))
