@@ -190,7 +190,11 @@ int32_t pic_sync(pic_ctx* ctx);
  * frames / exchange-buffer entries / frame-table entries below what the workspace was sized for; only before the
  * first pic_load_particles; the step then raises PIC_DEV_FRAME_POOL_EXHAUSTED / PIC_DEV_EXCHANGE_OVERFLOW /
  * PIC_DEV_TABLE_POOL_EXHAUSTED instead of writing out of bounds),
- * key "yee_tile" (8 or 16, default 8: y extent of the field-update kernel's 32-wide tile; same results),
+ * key "yee_tile" (8 or 16: y extent of the field-update kernel's tile; 0 = the measured best of the kernel in use,
+ * default; same results),
+ * key "yee_wide" (1 = on grids at least 64 cells wide along x the field update runs the kernel with four cells per
+ * thread and 16-byte accesses — default; 0 = always the kernel with one cell per thread, which narrower grids get
+ * anyway; same results to rounding order),
  * key "yee_index64" (1 = the field-update kernel indexes with 64 bits, as it does by itself once the padded six-component
  * array exceeds 2^32 elements; default 0; same results),
  * key "class_all" (-1 = decide from the population counters read at the last synchronisation which kernel

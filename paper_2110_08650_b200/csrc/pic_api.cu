@@ -29,7 +29,7 @@ struct pic_ctx {
     float* Fbuf[2];              // the two PADDED field buffers (periodic halos pre-filled); d.Fpad == Fbuf[F_cur]
     int F_cur;
     bool yee_index64;            // option "yee_index64": force the 64-bit-index instantiation (taken anyway beyond 2^32 elements)
-    int yee_tile;                // option "yee_tile": y extent of the Yee kernel's tile (8 or 16)
+    int yee_tile;                // option "yee_tile": y extent of the Yee kernel's tile (8 or 16; 0 = the measured best)
     bool yee_wide;               // option "yee_wide": four cells per thread where the grid is at least 64 wide (default)
     bool dirty;                  // pool cur holds a stepped state whose sort is still pending
     bool sparse_nosort;          // option "sparse_nosort": all-sparse steps skip the re-sort (default on)
@@ -449,7 +449,7 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     c->sparse_nosort = true;
     c->steps_unsorted = 0;
     c->field_update = false;
-    c->yee_tile = 8;
+    c->yee_tile = 0;
     c->yee_wide = true;
     c->yee_index64 = false;
     c->dirty = false;
@@ -873,7 +873,7 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
     if (!strcmp(key, "yee_index64")) { c->yee_index64 = value != 0; return PIC_OK; }
     if (!strcmp(key, "yee_wide")) { c->yee_wide = value != 0; return PIC_OK; }
     if (!strcmp(key, "yee_tile")) {
-        if (value != 8 && value != 16) return fail(c, PIC_EINVAL, "pic_set_option: yee_tile must be 8 or 16");
+        if (value != 0 && value != 8 && value != 16) return fail(c, PIC_EINVAL, "pic_set_option: yee_tile must be 0, 8 or 16");
         c->yee_tile = (int)value;
         return PIC_OK;
     }
