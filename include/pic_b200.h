@@ -102,8 +102,9 @@ int32_t pic_load_particles(pic_ctx* ctx, int64_t n,
                            const float* ux, const float* uy, const float* uz,
                            const float* w, const int32_t* species);
 
-/* Set the fields ("pic_set_fields(E,B)"): six float32 grid arrays, copied into the workspace
- * (asynchronous).  They stay as set (static external fields, the contract's five configs) unless
+/* Set the fields ("pic_set_fields(E,B)"): six float32 grid arrays [nz][ny][nx], copied into the workspace
+ * by one kernel (asynchronous) — the workspace keeps them in one array padded with their periodic images, the form
+ * the step kernel's TMA loads and the field update read and write.  They stay as set (static external fields, the contract's five configs) unless
  * pic_update_fields / option "field_update" advances them. */
 int32_t pic_set_fields(pic_ctx* ctx, const float* Ex, const float* Ey, const float* Ez,
                        const float* Bx, const float* By, const float* Bz);
@@ -129,8 +130,8 @@ int32_t pic_step(pic_ctx* ctx, int32_t n);
  * pic_step(n) ends with it.  Asynchronous; PIC_ESTATE before pic_set_fields. */
 int32_t pic_update_fields(pic_ctx* ctx);
 
-/* Copy the current E, B out: six float32 grid arrays (any may be NULL).  Asynchronous
- * device-to-device copies on the stream; PIC_ESTATE before pic_set_fields. */
+/* Copy the current E, B out: six float32 grid arrays [nz][ny][nx] (any may be NULL).  One kernel on the
+ * stream (asynchronous); PIC_ESTATE before pic_set_fields. */
 int32_t pic_get_fields(pic_ctx* ctx, float* Ex, float* Ey, float* Ez, float* Bx, float* By, float* Bz);
 
 /* Copy the last step's J ("pic_get_current"), periodic-folded, three float32 grid
