@@ -196,6 +196,9 @@ int32_t pic_sync(pic_ctx* ctx);
  * key "yee_wide" (1 = on grids at least 64 cells wide along x the field update runs the kernel with four cells per
  * thread and 16-byte accesses — default; 0 = always the kernel with one cell per thread, which narrower grids get
  * anyway; same results to rounding order),
+ * key "overlap" (1 = the two dense variants of a step, which take disjoint supercells, are launched side by side —
+ * the crowded supercells' one on a second stream the context owns, forked from and joined to the context's stream by
+ * events, so the stream order the caller sees is unchanged; default.  0 = one after the other.  Same results),
  * key "yee_index64" (1 = the field-update kernel indexes with 64 bits, as it does by itself once the padded six-component
  * array exceeds 2^32 elements; default 0; same results),
  * key "class_all" (-1 = decide from the population counters read at the last synchronisation which kernel

@@ -30,6 +30,8 @@ struct pic_ctx {
     int F_cur;
     bool yee_index64;            // option "yee_index64": force the 64-bit-index instantiation (taken anyway beyond 2^32 elements)
     int yee_tile;                // option "yee_tile": y extent of the Yee kernel's tile (8 or 16; 0 = the measured best)
+    PicAux aux;                  // second stream for the crowded supercells' variant (option "overlap"), with its events
+    bool overlap;
     bool yee_wide;               // option "yee_wide": four cells per thread where the grid is at least 64 wide (default)
     bool dirty;                  // pool cur holds a stepped state whose sort is still pending
     bool sparse_nosort;          // option "sparse_nosort": all-sparse steps skip the re-sort (default on)
@@ -450,6 +452,8 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     c->steps_unsorted = 0;
     c->field_update = false;
     c->yee_tile = 0;
+    c->aux = PicAux{nullptr, nullptr, nullptr};
+    c->overlap = true;
     c->yee_wide = true;
     c->yee_index64 = false;
     c->dirty = false;
@@ -522,6 +526,15 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
     if (e == cudaSuccess) e = cudaMemsetAsync(w + L.ctr, 0, L.Fpad - L.ctr, c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(w + L.J, 0, L.sc_offset - L.J, c->stream);
     if (e != cudaSuccess) { int r = cuda_fail(nullptr, e, "pic_create: cudaMemsetAsync"); delete c; return r; }
+    // second stream for the crowded supercells' variant; without it the variants run one after the other
+    if (cudaStreamCreateWithFlags(&c->aux.stream, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->aux.fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->aux.join, cudaEventDisableTiming) != cudaSuccess) {
+        cudaGetLastError();
+        if (c->aux.fork) cudaEventDestroy(c->aux.fork);
+        if (c->aux.stream) cudaStreamDestroy(c->aux.stream);
+        c->aux = PicAux{nullptr, nullptr, nullptr};
+    }
     *out = c;
     return PIC_OK;
 }
@@ -681,7 +694,8 @@ static int enqueue_steps(pic_ctx* c, int n, cudaStream_t st)
             ds.sort_filter = d.class_all == 1 ? 0 : 1;
             if (e == cudaSuccess) e = pic_launch_sort(ds, st, &c->launches);
         }
-        if (e == cudaSuccess) e = pic_launch_step(d, c->order, c->use_tma && c->tmap_ok, fix, c->tmap[c->F_cur], st, &c->launches, c->cell_kernel);
+        if (e == cudaSuccess) e = pic_launch_step(d, c->order, c->use_tma && c->tmap_ok, fix, c->tmap[c->F_cur], st, &c->launches, c->cell_kernel,
+                                                  c->overlap ? c->aux : PicAux{nullptr, nullptr, nullptr});
         d.fused = 0;
         if (e == cudaSuccess && c->timing) {
             e = cudaEventRecord(ev1, st);
@@ -872,6 +886,7 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
     }
     if (!strcmp(key, "yee_index64")) { c->yee_index64 = value != 0; return PIC_OK; }
     if (!strcmp(key, "yee_wide")) { c->yee_wide = value != 0; return PIC_OK; }
+    if (!strcmp(key, "overlap")) { c->overlap = value != 0; return PIC_OK; }
     if (!strcmp(key, "yee_tile")) {
         if (value != 0 && value != 8 && value != 16) return fail(c, PIC_EINVAL, "pic_set_option: yee_tile must be 0, 8 or 16");
         c->yee_tile = (int)value;
@@ -931,6 +946,9 @@ int32_t pic_destroy(pic_ctx* c)
 {
     if (!c) return PIC_EINVAL;
     for (cudaEvent_t ev : c->events) cudaEventDestroy(ev);
+    if (c->aux.fork) cudaEventDestroy(c->aux.fork);
+    if (c->aux.join) cudaEventDestroy(c->aux.join);
+    if (c->aux.stream) cudaStreamDestroy(c->aux.stream);
     delete c;
     return PIC_OK;
 }

@@ -176,8 +176,11 @@ __host__ __device__ inline uint32_t pic_pack_bits(int local_cell, int species)
 }
 
 // launchers implemented in pic_step.cu
+// aux: a second stream with its fork/join events (or aux.stream == nullptr): the two dense variants, which take disjoint
+// supercells, then run side by side — the crowded supercells' few long CTAs first, the ordinary ones filling the SMs
+struct PicAux { cudaStream_t stream; cudaEvent_t fork, join; };
 cudaError_t pic_launch_step(const PicDev& d, int order, bool use_tma, bool fixed_point, const void* tmap,
-                            cudaStream_t st, int64_t* launches, int cell_kernel);
+                            cudaStream_t st, int64_t* launches, int cell_kernel, const PicAux& aux);
 // pic_cell.cu: the dense whole-cell kernel (fixed point), launched over all supercells; sparse ones exit
 cudaError_t pic_launch_cell(const PicDev& d, int order, bool use_tma, const void* tmap, cudaStream_t st, int64_t* launches,
                             bool persistent);

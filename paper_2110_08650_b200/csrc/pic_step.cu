@@ -919,11 +919,24 @@ static cudaError_t launch_step_one(const PicDev& d, const CUtensorMap& map, cuda
 }
 
 template <int O, bool TMA, bool FIX>
-static cudaError_t launch_step_variant(const PicDev& d, const CUtensorMap& map, cudaStream_t st, int64_t* launches, int cell)
+static cudaError_t launch_step_variant(const PicDev& d, const CUtensorMap& map, cudaStream_t st, int64_t* launches, int cell,
+                                       const PicAux& aux)
 {
     cudaError_t e = cudaSuccess;
     if (d.class_all != 1 && cell) {     // dense supercells: the whole-cell kernel of pic_cell.cu (fixed point only)
         e = pic_launch_cell(d, O, TMA, &map, st, launches, cell == 2);
+    } else if (d.class_all != 1 && d.two_phase && aux.stream) {
+        // Both dense variants, side by side: they take disjoint supercells and meet only in atomics (J, the exchange
+        // buffer, the frame stack, the counters).  The crowded supercells (one-phase variant: a few hundred CTAs that
+        // run for milliseconds and leave SMs idle at their end — profiles/README.md, hot-spot table) are launched first,
+        // on the second stream; the ordinary supercells' CTAs fill what they leave free.
+        e = cudaEventRecord(aux.fork, st);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(aux.stream, aux.fork, 0);
+        if (e == cudaSuccess) e = launch_step_one<O, TMA, FIX, PIC_MODE_ONE>(d, map, aux.stream);
+        if (e == cudaSuccess) e = launch_step_one<O, TMA, FIX, PIC_MODE_TWO>(d, map, st);
+        if (e == cudaSuccess) e = cudaEventRecord(aux.join, aux.stream);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(st, aux.join, 0);
+        *launches += 2;
     } else if (d.class_all != 1) {      // dense variants (none when the host knows every supercell to be sparse)
         if (d.two_phase) {
             e = launch_step_one<O, TMA, FIX, PIC_MODE_TWO>(d, map, st);
@@ -948,17 +961,17 @@ static cudaError_t launch_step_variant(const PicDev& d, const CUtensorMap& map, 
 }
 
 cudaError_t pic_launch_step(const PicDev& d, int order, bool use_tma, bool fixed_point, const void* tmap,
-                            cudaStream_t st, int64_t* launches, int cell_kernel)
+                            cudaStream_t st, int64_t* launches, int cell_kernel, const PicAux& aux)
 {
     const int cell = fixed_point ? cell_kernel : 0;
     CUtensorMap map;
     if (use_tma) memcpy(&map, tmap, sizeof map); else memset(&map, 0, sizeof map);
     cudaError_t e;
 #define PIC_GO(O)                                                                               \
-    e = use_tma ? (fixed_point ? launch_step_variant<O, true, true>(d, map, st, launches, cell)                 \
-                               : launch_step_variant<O, true, false>(d, map, st, launches, cell))               \
-                : (fixed_point ? launch_step_variant<O, false, true>(d, map, st, launches, cell)                \
-                               : launch_step_variant<O, false, false>(d, map, st, launches, cell))
+    e = use_tma ? (fixed_point ? launch_step_variant<O, true, true>(d, map, st, launches, cell, aux)                 \
+                               : launch_step_variant<O, true, false>(d, map, st, launches, cell, aux))               \
+                : (fixed_point ? launch_step_variant<O, false, true>(d, map, st, launches, cell, aux)                \
+                               : launch_step_variant<O, false, false>(d, map, st, launches, cell, aux))
     switch (order) {
         case 1: PIC_GO(1); break;
         case 2: PIC_GO(2); break;
