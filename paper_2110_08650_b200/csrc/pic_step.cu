@@ -92,6 +92,7 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
     float4* s_stgP = reinterpret_cast<float4*>(smem_raw + S::OFF_STGP);
     float* s_stgF = reinterpret_cast<float*>(smem_raw + S::OFF_STGF);
     __shared__ int s_xn, s_slown, s_xbase, s_next, s_nitems;
+    __shared__ int s_any;        // sparse variant: some particle of the supercell deposited
     __shared__ int s_tbl[two_phase ? (768 * PIC_ITEM_LMAX(O)) / PIC_FRAME + 3 : 1];
     __shared__ __align__(8) uint64_t s_bar;
 
@@ -147,6 +148,7 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
         s_xn = 0;
         s_slown = 0;
         s_next = 0;
+        s_any = 0;
     }
     __syncthreads();
     // work items: every cell is cut into k = ceil(n/T) near-equal segments, T ~ 3/4 of the mean cell
@@ -233,8 +235,10 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
             // a particle whose position did not change in fp32 deposits exactly nothing (every DS is 0): a warp of
             // such particles (cold plasma ahead of a laser pulse) skips the deposit altogether
             const bool moved = (x1[0] != f0[0]) | (x1[1] != f0[1]) | (x1[2] != f0[2]);
-            if (__any_sync(0xffffffffu, moved))
+            if (__any_sync(0xffffffffu, moved)) {
+                if (lane == 0) s_any = 1;
                 deposit_direct<O, FIX>(d, sJ, sJhi, sJlo, fix_scale, f0, x1, d.q[sp] * P.w, lc);
+            }
             if (active)
                 finish_particle(d, rec, idx, s, ssx, ssy, ssz, cx, cy, cz, sp, P, M, un, fn, sh, s_hist, &s_xn, s_xrec,
                                 s_xid, s_xdst);
@@ -518,7 +522,10 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
         if (s_hist[t] != 0) atomicAdd(d.cell_hist + (size_t)s * 256 + t, s_hist[t]);
 
     // ---- a4: flush the J tile once (periodic wrap on write)
-    {
+    // A sparse supercell none of whose particles moved (cold plasma ahead of a laser pulse) has an all-zero tile: no
+    // flush.  And a node is read before its address is worked out: at 1.5 particles per cell most nodes of a tile are
+    // zero, and the walk over the 3456 nodes was 38 % of the sparse variant's instructions on configs[2] (ncu).
+    if (!SPARSE || s_any) {
         const size_t ncell = (size_t)d.nx * d.ny * d.nz;
         // 16 lanes per tile row of JNX <= 13 nodes: the row's y/z wrap and component are worked out once per row
         constexpr int ROWS = 3 * G::JNZ * G::JNY;
@@ -527,6 +534,15 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
         if (i < G::JNX)
         for (int row = tid >> 4; row < ROWS; row += NT / 16) {
             const int e = row * G::JNX + i;
+            long long n = 0;
+            float v = 0.0f;
+            if (FIX) {
+                n = ((long long)sJhi[e] << PIC_FIX_LO_BITS) + (long long)sJlo[e];
+                if (n == 0) continue;
+            } else {
+                v = sJ[e];
+                if (v == 0.0f) continue;
+            }
             const int j = row % G::JNY;
             const int r2 = row / G::JNY;
             const int k = r2 % G::JNZ;
@@ -535,20 +551,15 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
             const size_t g = c * ncell + (size_t)gi + (size_t)d.nx * ((size_t)gj + (size_t)d.ny * gk);
             if (FIX) {
                 // 64-bit fixed point in global memory too (native RED.64 in L2)
-                const long long n = ((long long)sJhi[e] << PIC_FIX_LO_BITS) + (long long)sJlo[e];
-                if (n != 0) atomicAdd(reinterpret_cast<unsigned long long*>(d.J64) + g, (unsigned long long)n);
+                atomicAdd(reinterpret_cast<unsigned long long*>(d.J64) + g, (unsigned long long)n);
+            } else if (d.float_tile_to_j64) {
+                // float tile of a sparse supercell (few same-node collisions: the CAS loop of a float atomic is
+                // cheaper there than two integer atomics) into the fixed-point global accumulators
+                const float jfc = c == 0 ? d.jfx : c == 1 ? d.jfy : d.jfz;
+                const double scale = (double)fix_scale_of(d, jfc) * (double)(1 << PIC_FIX_LO_BITS);
+                atomicAdd(reinterpret_cast<unsigned long long*>(d.J64) + g, (unsigned long long)__double2ll_rn((double)v * scale));
             } else {
-                const float v = sJ[e];
-                if (v == 0.0f) continue;
-                if (d.float_tile_to_j64) {
-                    // float tile of a sparse supercell (few same-node collisions: the CAS loop of a float atomic is
-                    // cheaper there than two integer atomics) into the fixed-point global accumulators
-                    const float jfc = c == 0 ? d.jfx : c == 1 ? d.jfy : d.jfz;
-                    const double scale = (double)fix_scale_of(d, jfc) * (double)(1 << PIC_FIX_LO_BITS);
-                    atomicAdd(reinterpret_cast<unsigned long long*>(d.J64) + g, (unsigned long long)__double2ll_rn((double)v * scale));
-                } else {
-                    atomicAdd(d.J + g, v);
-                }
+                atomicAdd(d.J + g, v);
             }
         }
     }
