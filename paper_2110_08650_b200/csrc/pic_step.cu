@@ -528,13 +528,28 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
     // flush.  And a node is read before its address is worked out: at 1.5 particles per cell most nodes of a tile are
     // zero, and the walk over the 3456 nodes was 38 % of the sparse variant's instructions on configs[2] (ncu).
     if (!SPARSE || s_any) {
-        const size_t ncell = (size_t)d.nx * d.ny * d.nz;
-        // 16 lanes per tile row of JNX <= 13 nodes: the row's y/z wrap and component are worked out once per row
-        // (tried: (j, k, component) carried from row to row instead of divided out, 32-bit cell index — config 2
-        // 2.79 vs 2.74 ms, KHI 6.60 vs 6.45, hot-spot 8.00 vs 7.78: the three carried registers cost more than the divisions)
+        // A row of the tile (component, z, y) maps to a row of the global array: its cell offset — two divisions, two
+        // periodic wraps, three multiplications — is worked out once per row into a table (in the leaver staging area,
+        // free by now), not once per node: the per-node version spent 44 instructions behind every non-zero node
+        // (ncu, hot-spot variant: 228 of 2044 thread instructions per particle).  32-bit offsets: pic_create admits at
+        // most 2^22 supercells = 2^30 cells, and 3 x 2^30 < 2^32.
         constexpr int ROWS = 3 * G::JNZ * G::JNY;
+        static_assert(ROWS * 4 <= PIC_XSTAGE * 40, "row table must fit the leaver staging area");
+        unsigned* s_rowbase = reinterpret_cast<unsigned*>(smem_raw + S::OFF_XREC);
+        const unsigned ncell = (unsigned)d.nx * (unsigned)d.ny * (unsigned)d.nz;
+        __syncthreads();                 // the append above has read the staging area
+        for (int row = tid; row < ROWS; row += NT) {
+            const int j = row % G::JNY;
+            const int r2 = row / G::JNY;
+            const int k = r2 % G::JNZ;
+            const int c = r2 / G::JNZ;
+            const int gj = wrapi(oy + j - G::JL, d.ny), gk = wrapi(oz + k - G::JL, d.nz);
+            s_rowbase[row] = (unsigned)c * ncell + (unsigned)d.nx * ((unsigned)gj + (unsigned)d.ny * (unsigned)gk);
+        }
+        __syncthreads();
+        // 16 lanes per tile row of JNX <= 13 nodes
         const int i = tid & 15;
-        const int gi = wrapi(ox + i - G::JL, d.nx);
+        const unsigned gi = (unsigned)wrapi(ox + i - G::JL, d.nx);
         if (i < G::JNX)
         for (int row = tid >> 4; row < ROWS; row += NT / 16) {
             const int e = row * G::JNX + i;
@@ -547,18 +562,14 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
                 v = sJ[e];
                 if (v == 0.0f) continue;
             }
-            const int j = row % G::JNY;
-            const int r2 = row / G::JNY;
-            const int k = r2 % G::JNZ;
-            const int c = r2 / G::JNZ;
-            const int gj = wrapi(oy + j - G::JL, d.ny), gk = wrapi(oz + k - G::JL, d.nz);
-            const size_t g = c * ncell + (size_t)gi + (size_t)d.nx * ((size_t)gj + (size_t)d.ny * gk);
+            const size_t g = (size_t)(s_rowbase[row] + gi);
             if (FIX) {
                 // 64-bit fixed point in global memory too (native RED.64 in L2)
                 atomicAdd(reinterpret_cast<unsigned long long*>(d.J64) + g, (unsigned long long)n);
             } else if (d.float_tile_to_j64) {
                 // float tile of a sparse supercell (few same-node collisions: the CAS loop of a float atomic is
                 // cheaper there than two integer atomics) into the fixed-point global accumulators
+                const int c = row / (G::JNY * G::JNZ);
                 const float jfc = c == 0 ? d.jfx : c == 1 ? d.jfy : d.jfz;
                 const double scale = (double)fix_scale_of(d, jfc) * (double)(1 << PIC_FIX_LO_BITS);
                 atomicAdd(reinterpret_cast<unsigned long long*>(d.J64) + g, (unsigned long long)__double2ll_rn((double)v * scale));
