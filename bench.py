@@ -561,7 +561,7 @@ def main():
     ap.add_argument("--cell-kernel", type=int, default=0, help="1: dense supercells go to pic_cell_kernel (third generation), 0: round-1 kernels")
     ap.add_argument("--direct-below", type=int, default=768, help="supercells with fewer particles take the per-particle (sparse) kernel")
     ap.add_argument("--opt", action="append", default=[], help="key=value: any further pic_set_option (experiments)")
-    ap.add_argument("--sparse-nosort", type=int, default=1, help="1: all-sparse steps skip the re-sort (one sort in eight steps)")
+    ap.add_argument("--sparse-nosort", type=int, default=1, help="1: all-sparse steps skip the re-sort (one sort in 16 steps; N >= 2: one in N)")
     ap.add_argument("--crowd-first", type=int, default=0, help="1: the step kernels start crowded supercells first")
     ap.add_argument("--repeats", type=int, default=5, help="the headline is the median of this many runs, each from a fresh load")
     ap.add_argument("--late-run", type=int, default=1, help="1: also time the last 20 steps of the workload's own step count")

@@ -186,7 +186,8 @@ int32_t pic_sync(pic_ctx* ctx);
  * key "direct_below" (default 768: supercells with fewer particles take the one-thread-per-particle variant),
  * key "sparse_float" (1 = a step that only launches that variant accumulates J in float, default; 0 = always fixed point),
  * key "sparse_nosort" (1 = such a step also skips the re-sort of the previous step's result and walks the slots as they
- * are — holes of leavers, appended arrivals —, with one sort in eight steps; default; 0 = sort before every step),
+ * are — holes of leavers, appended arrivals —, with one sort in 16 steps; default; N >= 2 = the same with one sort in N
+ * steps; 0 = sort before every step),
  * keys "limit_frames", "limit_exchange", "limit_tables" (fault injection for tests: lower the number of particle
  * frames / exchange-buffer entries / frame-table entries below what the workspace was sized for; only before the
  * first pic_load_particles; the step then raises PIC_DEV_FRAME_POOL_EXHAUSTED / PIC_DEV_EXCHANGE_OVERFLOW /

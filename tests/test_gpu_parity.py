@@ -99,12 +99,13 @@ def test_energy_conserving_gather_variant(name):
     ref.destroy()
 
 
-@pytest.mark.parametrize("nosort", (0, 1))
+@pytest.mark.parametrize("nosort", (0, 1, 4))
 def test_all_sparse_steps_without_resort(nosort):
     """All-sparse workload (2 particles per cell, one thread per particle): with option sparse_nosort the steps run on
-    the unsorted state (holes of leavers, appended arrivals) and sort once in eight steps.  20 free-running steps of a
-    hot, sparse plasma (a few per cent of the particles change supercell per step, whole supercells of the slab
-    boundary empty and fill) against the oracle, with and without the option; read-backs in between sort on demand."""
+    the unsorted state (holes of leavers, appended arrivals) and sort once in 16 steps (option value 1) or in 4 (option
+    value 4: the periodic sort inside a pic_step(n) call, several times).  20 free-running steps of a hot, sparse
+    plasma (a few per cent of the particles change supercell per step, whole supercells of the slab boundary empty
+    and fill) against the oracle, with and without the option; read-backs in between sort on demand."""
     wl = W.CONFIGS["lwfa"].scaled((32, 64, 16), u_th=0.25, ramp_cells=8)
     parts, fields = W.make_particles(wl), W.make_fields(wl) * 0.02
     orc = PP.oracle_for(wl, parts, fields)
