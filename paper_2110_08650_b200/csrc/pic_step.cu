@@ -189,6 +189,16 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
         }
     }
 
+    // Sparse variant: is the staged E/B tile all zero (plasma the fields have not reached)?  A particle at rest
+    // (u = 0 exactly) in such a supercell gathers F = 0, keeps u = 0 and x, and deposits nothing: the step leaves its
+    // record bit for bit as it is, so only the cell histogram has to hear of it (see the particle loop).
+    bool tile_zero = false;
+    if (SPARSE) {
+        unsigned any = 0;
+        for (int e = tid; e < 6 * G::FCOMP; e += NT) any |= __float_as_uint(sF[e]) << 1;     // -0 counts as zero
+        tile_zero = __syncthreads_or(any != 0) == 0;
+    }
+
     float fix_scale[3] = {1.0f, 1.0f, 1.0f};
     if (FIX) {
         fix_scale[0] = fix_scale_of(d, d.jfx);
@@ -230,6 +240,12 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
             const uint32_t bits = __float_as_uint(M.w);
             const int lc = bits & 0xff, sp = (bits >> 16) & 0xff;
             const int cx = lc & 7, cy = (lc >> 3) & 7, cz = lc >> 6;
+            // a warp of particles at rest in a field-free supercell: nothing to compute, nothing to write back
+            const bool at_rest = tile_zero && ((__float_as_uint(M.x) | __float_as_uint(M.y) | __float_as_uint(M.z)) << 1) == 0;
+            if (__all_sync(0xffffffffu, at_rest || !active)) {
+                if (active) atomicAdd(&s_hist[lc], 1);
+                continue;
+            }
             float un[3], fn[3], x1[3];
             int sh[3];
             push_particle<O>(d, sF, cx, cy, cz, sp, P, M, un, fn, x1, sh);
