@@ -197,6 +197,9 @@ int32_t pic_sync(pic_ctx* ctx);
  * key "yee_wide" (1 = on grids at least 64 cells wide along x the field update runs the kernel with four cells per
  * thread and 16-byte accesses — default; 0 = always the kernel with one cell per thread, which narrower grids get
  * anyway; same results to rounding order),
+ * key "rest_skip" (1 = in the one-thread-per-particle variant a warp whose particles are all at rest, u = 0 exactly,
+ * in a supercell whose staged E/B tile is all zero skips gather, push, deposit and write-back — the step would rewrite
+ * their records bit for bit; default.  0 = every particle is stepped.  Bit-identical results: tests compare the two),
  * key "overlap" (1 = the two dense variants of a step, which take disjoint supercells, are launched side by side —
  * the crowded supercells' one on a second stream the context owns, forked from and joined to the context's stream by
  * events, so the stream order the caller sees is unchanged; default.  0 = one after the other.  Same results),

@@ -517,6 +517,7 @@ int32_t pic_create(pic_ctx** out, const int32_t grid[3], const double cell[3], d
         d.crowd_min = 1 << 30;
         d.direct_below = PIC_DIRECT_BELOW;
         d.gather_ec = 0;
+        d.rest_skip = 1;
         d.nosort = 0;
         d.sparse_float_tile = 0;
         d.float_tile_to_j64 = 0;
@@ -911,6 +912,7 @@ int32_t pic_set_option(pic_ctx* c, const char* key, int64_t value)
     if (!strcmp(key, "yee_index64")) { c->yee_index64 = value != 0; return PIC_OK; }
     if (!strcmp(key, "yee_wide")) { c->yee_wide = value != 0; return PIC_OK; }
     if (!strcmp(key, "overlap")) { c->overlap = value != 0; return PIC_OK; }
+    if (!strcmp(key, "rest_skip")) { c->d.rest_skip = value != 0; return PIC_OK; }
     if (!strcmp(key, "yee_tile")) {
         if (value != 0 && value != 8 && value != 16) return fail(c, PIC_EINVAL, "pic_set_option: yee_tile must be 0, 8 or 16");
         c->yee_tile = (int)value;

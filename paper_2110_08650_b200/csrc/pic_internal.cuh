@@ -93,6 +93,7 @@ struct PicDev {
     int sparse_float_tile;       // option "sparse_float_tile": the sparse variant keeps a float J tile (flushed into J64)
     int float_tile_to_j64;       // set by the launcher for that variant
     int nosort;                  // this step runs on the unsorted state of the last one (all-sparse steps, option "sparse_nosort")
+    int rest_skip;               // option "rest_skip": sparse variant, warps of particles at rest in a field-free supercell skip the particle
     int gather_ec;               // option "gather" = 1: energy-conserving gather (per-particle gather paths only)
     int direct_below;            // supercells with fewer particles count as sparse (one thread per particle); option "direct_below"
     int class_all;               // host's belief, from counters read at its last synchronisation (performance only, any

@@ -193,7 +193,7 @@ pic_step_kernel(const PicDev d, const __grid_constant__ CUtensorMap tmap)
     // (u = 0 exactly) in such a supercell gathers F = 0, keeps u = 0 and x, and deposits nothing: the step leaves its
     // record bit for bit as it is, so only the cell histogram has to hear of it (see the particle loop).
     bool tile_zero = false;
-    if (SPARSE) {
+    if (SPARSE && d.rest_skip) {
         unsigned any = 0;
         for (int e = tid; e < 6 * G::FCOMP; e += NT) any |= __float_as_uint(sF[e]) << 1;     // -0 counts as zero
         tile_zero = __syncthreads_or(any != 0) == 0;

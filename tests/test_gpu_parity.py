@@ -68,6 +68,34 @@ def test_dense_kernel_generations(name, kernel):
     pic.destroy()
 
 
+def test_particles_at_rest_in_field_free_supercells_are_skipped_exactly():
+    """configs[2] shape: cold plasma (u = 0 exactly) and a laser pulse that underflows to exact zeros away from its
+    centre.  The one-thread-per-particle variant skips warps of particles at rest in supercells whose E/B tile is all
+    zero (option rest_skip, default on); with the option off every particle is stepped.  Positions, momenta and J after 6
+    steps must agree bit for bit (J in fixed point, sparse_float = 0: the float accumulation of all-sparse steps depends
+    on the order of its atomics), and the case must contain both kinds of particle."""
+    wl = W.CONFIGS["lwfa"].scaled((16, 512, 8))      # long enough along y for the pulse (w_y = 16 cells) to die out
+    parts, fields = W.make_particles(wl), W.make_fields(wl)
+    assert float(parts.ux.abs().max()) == 0.0 and float(parts.uy.abs().max()) == 0.0     # cold start
+    nz_planes = (fields.abs().amax(dim=(0, 1, 3)) > 0).sum().item()
+    assert 0 < nz_planes < wl.grid[1] - 16          # the pulse covers part of y only: field-free supercells exist
+    out = []
+    for skip in (1, 0):
+        pic = PP.gpu_for(wl, parts, fields, rest_skip=skip, sparse_float=0)
+        pic.step(6)
+        pic.sync()
+        assert pic.get_stats()["error"] == 0
+        out.append((PP.gpu_particles_by_id(pic), pic.get_current().cpu()))
+        pic.destroy()
+    (A, JA), (B, JB) = out
+    for k in ("x", "y", "z", "ux", "uy", "uz"):
+        assert np.array_equal(A[k], B[k]), k
+    assert torch.equal(JA, JB)
+    moved = np.abs(A["uy"]).max() > 0 or np.abs(A["ux"]).max() > 0
+    at_rest = ((A["ux"] == 0) & (A["uy"] == 0) & (A["uz"] == 0)).mean()
+    assert moved and 0.2 < at_rest < 1.0, at_rest
+
+
 @pytest.mark.parametrize("name", ["cfg1_tiny_cic", "cfg2_thermal_tsc_32", "cfg3_lwfa_tsc_32x128x32", "cfg5_pqs_32x32x16"])
 def test_energy_conserving_gather_variant(name):
     """Option gather = 1 against the oracle's energy-conserving gather (pinned in
