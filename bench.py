@@ -341,6 +341,8 @@ def measure_other(args, wl, dev, peak):
             "leavers_per_step": st["leavers_last"], "max_supercell_population": st["max_count"], "error_word": st["error"],
             "field_update_ms": fu_ms,
             "field_update_frac_60B": FIELD_UPDATE_BYTES_PER_CELL * wl.n_cells / (fu_ms * 1e-3) / 1e9 / peak,
+            "exact_shortcuts": "sparse supercells only (option rest_skip, default on; results bit-identical, tested): warps of "
+                               "particles at rest in a supercell whose E/B tile is all zero are not stepped",
             "load_and_setup_s": t_load}
 
 
